@@ -1,0 +1,140 @@
+/*
+ * fbp.h -- C ABI of libfbp: 2-D parallel-beam filtered back-projection on one B200 (sm_100a).
+ *
+ * The operation is the one the paper states (arxiv 2109.02174, "PAPER.md"):
+ *   PAPER.md:55   a ray is  x cos(theta) + y sin(theta) = t;  the projections P_theta(t)
+ *                 indexed by (angle, detector offset) form the sinogram.
+ *   PAPER.md:61   Q_theta(t) = P_theta(t) * H(t)               -- the filter step
+ *   PAPER.md:59   f(x,y) = sum_i Q_theta_i( x cos theta_i + y sin theta_i )   (eq. 2)
+ * The paper leaves the filter, the interpolation and the scale factors open; the readings
+ * taken are:
+ *   taps   h[0] = 1/4,  h[m] = -1/(pi^2 m^2) for odd m,  0 for even m != 0      (Ram-Lak)
+ *   filter Q[i][n] = (1/d) * sum_{k=0}^{D-1} h[n-k] P[i][k]      (linear, "same", zero-extended)
+ *   pixel  x = (c - (N-1)/2) * pix,  y = (r - (N-1)/2) * pix     (column <-> +x, row <-> +y)
+ *   coord  u = (x cos theta_i + y sin theta_i)/d + (D-1)/2 ;  j = floor(u) ;  w = u - j
+ *   interp q_i = (1-w) Q~[i][j] + w Q~[i][j+1],   Q~ = 0 outside [0, D-1]
+ *   image  f[r][c] = (pi/K) * sum_{i=0}^{K-1} q_i                (every angle weighted pi/K)
+ *
+ * Conventions common to every entry point
+ *   - Arrays are dense, row-major, element type = the plan's dtype (float or double):
+ *       sinogram / filtered sinogram  [batch][n_angles][n_det]
+ *       image                         [batch][image_n][image_n]
+ *   - "d_" arguments are DEVICE pointers (16-byte aligned), "h_" arguments are HOST pointers.
+ *     The caller owns them; inputs are never written; outputs are fully overwritten.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *     Device-pointer calls only enqueue work on that stream: no host synchronisation, no
+ *     allocation.  A plan must not be used from two streams at once (it owns scratch
+ *     buffers); different plans are independent.
+ *   - Determinism: every output element has one owner thread and a fixed summation order
+ *     (no atomics, no read-modify-write between threads -- the defect PAPER.md:218 reports
+ *     for its parallel versions).  Same plan parameters + same input bytes => same output
+ *     bytes on every run.
+ *   - Errors: a non-zero fbp_status is returned, nothing is enqueued and no output is
+ *     touched.  FBP_EINVAL: NULL / misaligned pointers, sizes out of range, non-finite
+ *     geometry, batch < 1 or > max_batch.  FBP_ENOMEM: allocation failure.
+ *     FBP_EUNSUPPORTED: the device is not compute capability 10.x (there is no fallback
+ *     path by design).  FBP_ECUDA: any CUDA runtime error (text via fbp_last_error).
+ *     Nothing throws across this boundary and nothing calls exit/abort.
+ */
+#ifndef FBP_H_
+#define FBP_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fbp_plan fbp_plan; /* opaque; owned by the library */
+
+typedef enum { FBP_F32 = 0, FBP_F64 = 1 } fbp_dtype;
+
+typedef enum {
+    FBP_OK = 0,
+    FBP_EINVAL = 1,
+    FBP_ENOMEM = 2,
+    FBP_ECUDA = 3,
+    FBP_EUNSUPPORTED = 4
+} fbp_status;
+
+/*
+ * fbp_create -- build a plan for one geometry (rays x cos + y sin = t).
+ *   out          receives the plan (HOST pointer to a pointer); NULL on failure
+ *   n_angles     K >= 1;  n_det  D >= 2
+ *   angles_rad   HOST pointer, K finite values theta_i in radians; copied
+ *   det_spacing  d > 0; the detector is centred: t_j = (j - (D-1)/2) * d
+ *   image_n      N >= 1;  pixel_size > 0, or <= 0 meaning "= det_spacing"
+ *   dtype        arithmetic and storage type of every array passed to this plan
+ *   max_batch    >= 1; sizes the plan-owned filtered-sinogram scratch used by fbp_reconstruct
+ *   device       CUDA ordinal, or -1 for the current device
+ * Host work happens here only: the Ram-Lak taps and the cos/sin table are computed in fp64
+ * on the host and uploaded; scratch buffers are allocated.  Synchronous.
+ */
+fbp_status fbp_create(fbp_plan **out, int n_angles, int n_det, const double *angles_rad,
+                      double det_spacing, int image_n, double pixel_size, fbp_dtype dtype,
+                      int max_batch, int device);
+
+/*
+ * fbp_filter -- Q = (1/d) h * P along the detector axis of every row.
+ *   d_sino [batch][K][D] in, d_filtered [batch][K][D] out (may not alias).
+ */
+fbp_status fbp_filter(fbp_plan *plan, const void *d_sino, void *d_filtered, int batch,
+                      void *cuda_stream);
+
+/*
+ * fbp_backproject -- f = (pi/K) sum_i lerp(Q_i, u_i(x,y)) for every pixel (eq. 2).
+ *   d_filtered [batch][K][D] in, d_image [batch][N][N] out.  Includes the pi/K weight.
+ */
+fbp_status fbp_backproject(fbp_plan *plan, const void *d_filtered, void *d_image, int batch,
+                           void *cuda_stream);
+
+/*
+ * fbp_reconstruct -- fbp_backproject(fbp_filter(sino)) through the plan-owned scratch;
+ * bit-identical to calling the two entry points in sequence.
+ */
+fbp_status fbp_reconstruct(fbp_plan *plan, const void *d_sino, void *d_image, int batch,
+                           void *cuda_stream);
+
+/*
+ * fbp_reconstruct_host -- the same reconstruction for HOST buffers: copies h_sino
+ * [batch][K][D] to a plan-owned device buffer, runs fbp_reconstruct, copies the image
+ * back to h_image [batch][N][N], and waits for the stream.  Pinned host memory makes the
+ * copies asynchronous until the final wait; pageable memory works too.  This is the
+ * end-to-end path bench.py's "e2e" leg times (copies inside the timed region).
+ */
+fbp_status fbp_reconstruct_host(fbp_plan *plan, const void *h_sino, void *h_image, int batch,
+                                void *cuda_stream);
+
+/* fbp_destroy -- free the plan, its tables and scratch.  NULL-safe.  Synchronous. */
+void fbp_destroy(fbp_plan *plan);
+
+/*
+ * fbp_last_error -- text of the last error on this plan (plan-owned, never freed by the
+ * caller; "" if none).  NULL plan: the last fbp_create error of the calling thread.
+ */
+const char *fbp_last_error(const fbp_plan *plan);
+
+/*
+ * fbp_plan_info -- launch configuration chosen by fbp_create, for tests, bench.py and
+ * DESIGN.md tables.  Writes up to `n` ints into `out` (HOST) and returns how many it has:
+ *   [0] back-projection tile width   [1] tile height   [2] pixels per thread (register tile)
+ *   [3] angle splits S (deterministic fixed-order reduction when > 1)
+ *   [4] angles staged per shared-memory chunk   [5] staged segment length (entries per angle)
+ *   [6] back-projection CTAs per slice   [7] back-projection threads per CTA
+ *   [8] back-projection dynamic shared memory bytes per CTA
+ *   [9] filter outputs per thread   [10] filter threads per CTA   [11] filter rows per CTA
+ *   [12] filter dynamic shared memory bytes per CTA   [13] kernels launched by fbp_reconstruct
+ */
+int fbp_plan_info(const fbp_plan *plan, int *out, int n);
+
+/*
+ * fbp_set_profiling / fbp_get_kernel_ms -- optional per-kernel timing of the LAST compute
+ * call, with CUDA events recorded on the caller's stream around each kernel group.
+ * fbp_get_kernel_ms waits for those events (host sync) and returns milliseconds; a group
+ * that did not run in the last call reports 0.  Off by default (no events recorded).
+ */
+fbp_status fbp_set_profiling(fbp_plan *plan, int enable);
+fbp_status fbp_get_kernel_ms(fbp_plan *plan, float *filter_ms, float *backproject_ms);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FBP_H_ */

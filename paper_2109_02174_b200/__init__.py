@@ -1,1 +1,92 @@
-"""B200-native parallel-beam filtered back-projection (arxiv 2109.02174 hot path)."""
+"""B200-native parallel-beam filtered back-projection (arxiv 2109.02174 hot path).
+
+The product is ``libfbp.so`` (C ABI in ``include/fbp.h``, kernels in ``csrc/``); this
+package is its ctypes binding plus the seeded input generators (``inputs``).  Nothing
+here computes any step of the method on the CPU and nothing imports ``oracle/``.
+"""
+from __future__ import annotations
+
+from .binding import (  # noqa: F401
+    EXPORTS, FBP_F32, FBP_F64, FBP_OK, FBP_EINVAL, FBP_ENOMEM, FBP_ECUDA, FBP_EUNSUPPORTED,
+    FbpError, load_library,
+    fbp_create, fbp_filter, fbp_backproject, fbp_reconstruct, fbp_reconstruct_host,
+    fbp_destroy, fbp_last_error, fbp_plan_info, fbp_set_profiling, fbp_get_kernel_ms,
+)
+from .build import build  # noqa: F401
+
+_DTYPES = {"f32": FBP_F32, "f64": FBP_F64, "float32": FBP_F32, "float64": FBP_F64}
+
+
+def shard_slices(n_slices: int, rank: int, world_size: int) -> range:
+    """Slices [lo, hi) of a stack owned by ``rank``: contiguous, balanced, no overlap.
+
+    Slices are independent problems (a volume is a stack of 2-D slices), so
+    multi-GPU runs shard them with no data-path collective (option 1)."""
+    if world_size < 1 or not 0 <= rank < world_size:
+        raise ValueError("bad rank/world_size")
+    base, rem = divmod(n_slices, world_size)
+    lo = rank * base + min(rank, rem)
+    return range(lo, lo + base + (1 if rank < rem else 0))
+
+
+class Plan:
+    """RAII wrapper over an ``fbp_plan*`` taking torch CUDA tensors (marshalling only)."""
+
+    def __init__(self, angles_rad, n_det, image_n, det_spacing=1.0, pixel_size=0.0, dtype="f32",
+                 max_batch=1, device=-1):
+        import torch
+        self.torch_dtype = torch.float32 if _DTYPES[dtype] == FBP_F32 else torch.float64
+        self.n_angles, self.n_det, self.image_n, self.max_batch = len(angles_rad), int(n_det), int(image_n), int(max_batch)
+        self.device = torch.device("cuda", torch.cuda.current_device() if device < 0 else device)
+        self.handle = fbp_create(self.n_angles, n_det, angles_rad, det_spacing, image_n, pixel_size,
+                                 _DTYPES[dtype], max_batch, device)
+
+    def info(self) -> dict:
+        return fbp_plan_info(self.handle)
+
+    def _batch(self, t, inner):
+        if t.dtype != self.torch_dtype or not t.is_cuda or not t.is_contiguous():
+            raise ValueError("expected a contiguous CUDA tensor of the plan dtype")
+        if tuple(t.shape[-2:]) != inner or t.dim() not in (2, 3):
+            raise ValueError("expected shape [batch]%s, got %s" % (list(inner), list(t.shape)))
+        return 1 if t.dim() == 2 else t.shape[0]
+
+    def _empty(self, like, inner):
+        import torch
+        shape = inner if like.dim() == 2 else (like.shape[0],) + inner
+        return torch.empty(shape, dtype=self.torch_dtype, device=like.device)
+
+    def filter(self, sino, out=None, stream=None):
+        b = self._batch(sino, (self.n_angles, self.n_det))
+        out = self._empty(sino, (self.n_angles, self.n_det)) if out is None else out
+        fbp_filter(self.handle, sino, out, b, stream)
+        return out
+
+    def backproject(self, filtered, out=None, stream=None):
+        b = self._batch(filtered, (self.n_angles, self.n_det))
+        out = self._empty(filtered, (self.image_n, self.image_n)) if out is None else out
+        fbp_backproject(self.handle, filtered, out, b, stream)
+        return out
+
+    def reconstruct(self, sino, out=None, stream=None):
+        b = self._batch(sino, (self.n_angles, self.n_det))
+        out = self._empty(sino, (self.image_n, self.image_n)) if out is None else out
+        fbp_reconstruct(self.handle, sino, out, b, stream)
+        return out
+
+    def close(self):
+        if getattr(self, "handle", None):
+            fbp_destroy(self.handle)
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

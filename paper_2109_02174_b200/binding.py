@@ -1,0 +1,161 @@
+"""ctypes binding of libfbp (include/fbp.h): argument marshalling only.
+
+Every step of the path (filter, then back-projection) runs in the CUDA
+kernels of ``csrc/``.  There is no CPU fallback: if ``libfbp.so`` is missing or fails to
+load, ``load_library`` raises.  torch is used for device memory and streams only.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+from . import build as _build
+
+FBP_F32, FBP_F64 = 0, 1
+FBP_OK, FBP_EINVAL, FBP_ENOMEM, FBP_ECUDA, FBP_EUNSUPPORTED = 0, 1, 2, 3, 4
+STATUS_NAMES = {0: "FBP_OK", 1: "FBP_EINVAL", 2: "FBP_ENOMEM", 3: "FBP_ECUDA", 4: "FBP_EUNSUPPORTED"}
+
+EXPORTS = (
+    "fbp_create", "fbp_filter", "fbp_backproject", "fbp_reconstruct", "fbp_reconstruct_host",
+    "fbp_destroy", "fbp_last_error", "fbp_plan_info", "fbp_set_profiling", "fbp_get_kernel_ms",
+)
+
+PLAN_INFO_FIELDS = (
+    "bp_tile_w", "bp_tile_h", "bp_pixels_per_thread", "bp_angle_splits", "bp_angles_per_chunk",
+    "bp_segment_len", "bp_ctas_per_slice", "bp_threads", "bp_smem_bytes",
+    "filter_outputs_per_thread", "filter_threads", "filter_rows_per_cta", "filter_smem_bytes",
+    "kernels_per_reconstruct",
+)
+
+_lib = None
+
+
+class FbpError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__("%s: %s" % (STATUS_NAMES.get(status, status), message))
+        self.status = status
+
+
+def load_library(path: str | None = None) -> ctypes.CDLL:
+    """Load libfbp.so (built in-tree by ``build.build()``); raise if it is not there."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    path = path or _build.LIB
+    if not os.path.exists(path):
+        raise FileNotFoundError(
+            "%s not found: build it with `python -m paper_2109_02174_b200.build` "
+            "(there is no CPU fallback)" % path)
+    lib = ctypes.CDLL(path)
+    vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+    lib.fbp_create.argtypes = [ctypes.POINTER(vp), ci, ci, ctypes.POINTER(cd), cd, ci, cd, ci, ci, ci]
+    lib.fbp_create.restype = ci
+    for name in ("fbp_filter", "fbp_backproject", "fbp_reconstruct", "fbp_reconstruct_host"):
+        fn = getattr(lib, name)
+        fn.argtypes = [vp, vp, vp, ci, vp]
+        fn.restype = ci
+    lib.fbp_destroy.argtypes = [vp]
+    lib.fbp_destroy.restype = None
+    lib.fbp_last_error.argtypes = [vp]
+    lib.fbp_last_error.restype = ctypes.c_char_p
+    lib.fbp_plan_info.argtypes = [vp, ctypes.POINTER(ci), ci]
+    lib.fbp_plan_info.restype = ci
+    lib.fbp_set_profiling.argtypes = [vp, ci]
+    lib.fbp_set_profiling.restype = ci
+    lib.fbp_get_kernel_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float)]
+    lib.fbp_get_kernel_ms.restype = ci
+    _lib = lib
+    return lib
+
+
+def _check(lib, plan, status: int):
+    if status != FBP_OK:
+        msg = lib.fbp_last_error(plan)
+        raise FbpError(status, msg.decode() if msg else "")
+
+
+def _ptr(x) -> int:
+    """Device/host address of a torch tensor, numpy array or a raw integer address."""
+    if x is None:
+        return 0
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    return x.ctypes.data
+
+
+def _stream_handle(stream) -> int:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+# ---- the C entry points, same names, same order of arguments -------------------------
+
+def fbp_create(n_angles, n_det, angles_rad, det_spacing, image_n, pixel_size, dtype, max_batch=1, device=-1):
+    """fbp_create of include/fbp.h; returns the opaque plan handle (an int address)."""
+    lib = load_library()
+    if angles_rad is None:
+        arr = None
+    else:
+        vals = [float(a) for a in angles_rad]
+        arr = (ctypes.c_double * max(len(vals), 1))(*vals)
+    plan = ctypes.c_void_p()
+    st = lib.fbp_create(ctypes.byref(plan), int(n_angles), int(n_det), arr, float(det_spacing), int(image_n),
+                        float(pixel_size), int(dtype), int(max_batch), int(device))
+    _check(lib, None, st)
+    return plan.value
+
+
+def fbp_filter(plan, d_sino, d_filtered, batch, stream=None):
+    lib = load_library()
+    _check(lib, plan, lib.fbp_filter(plan, _ptr(d_sino), _ptr(d_filtered), int(batch), _stream_handle(stream)))
+
+
+def fbp_backproject(plan, d_filtered, d_image, batch, stream=None):
+    lib = load_library()
+    _check(lib, plan, lib.fbp_backproject(plan, _ptr(d_filtered), _ptr(d_image), int(batch), _stream_handle(stream)))
+
+
+def fbp_reconstruct(plan, d_sino, d_image, batch, stream=None):
+    lib = load_library()
+    _check(lib, plan, lib.fbp_reconstruct(plan, _ptr(d_sino), _ptr(d_image), int(batch), _stream_handle(stream)))
+
+
+def fbp_reconstruct_host(plan, h_sino, h_image, batch, stream=None):
+    lib = load_library()
+    _check(lib, plan, lib.fbp_reconstruct_host(plan, _ptr(h_sino), _ptr(h_image), int(batch), _stream_handle(stream)))
+
+
+def fbp_destroy(plan):
+    if plan:
+        load_library().fbp_destroy(plan)
+
+
+def fbp_last_error(plan=None) -> str:
+    msg = load_library().fbp_last_error(plan)
+    return msg.decode() if msg else ""
+
+
+def fbp_plan_info(plan) -> dict:
+    lib = load_library()
+    n = len(PLAN_INFO_FIELDS)
+    buf = (ctypes.c_int * n)()
+    got = lib.fbp_plan_info(plan, buf, n)
+    return {PLAN_INFO_FIELDS[i]: int(buf[i]) for i in range(min(n, got))}
+
+
+def fbp_set_profiling(plan, enable: bool):
+    lib = load_library()
+    _check(lib, plan, lib.fbp_set_profiling(plan, 1 if enable else 0))
+
+
+def fbp_get_kernel_ms(plan):
+    lib = load_library()
+    f, b = ctypes.c_float(), ctypes.c_float()
+    _check(lib, plan, lib.fbp_get_kernel_ms(plan, ctypes.byref(f), ctypes.byref(b)))
+    return f.value, b.value

@@ -1,0 +1,503 @@
+// fbp.cu -- libfbp: plan, launch configuration and the C ABI of include/fbp.h.
+// Kernels: fbp_filter.cuh and fbp_backproject.cuh (eq. 2).
+// This library has no CPU path and shares nothing with oracle/ (the test oracle).
+#include "../../include/fbp.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "fbp_backproject.cuh"
+#include "fbp_filter.cuh"
+
+namespace {
+
+constexpr double kPi = 3.14159265358979323846264338327950288;
+constexpr int kNumSm = 148;  // B200
+
+thread_local std::string g_create_error;
+
+int env_int(const char* name, int dflt)
+{
+    const char* v = std::getenv(name);
+    if (!v || !*v) return dflt;
+    return std::atoi(v);
+}
+
+}  // namespace
+
+struct fbp_plan {
+    fbp_dtype dtype = FBP_F32;
+    int K = 0, D = 0, N = 0, max_batch = 0, device = 0;
+    double d = 1.0, pix = 1.0;
+    size_t esize = 4;
+
+    // device tables / scratch
+    double2* d_cs2 = nullptr;   // [K] (cos, sin) * pix/d, fp64
+    void* d_taps = nullptr;     // [tab_len] dtype
+    void* d_qwork = nullptr;    // [max_batch][K][D] filtered sinogram (fbp_reconstruct)
+    void* d_part = nullptr;     // [S][max_batch][N][N] partial images when S > 1
+    void* d_hsino = nullptr;    // host-path staging (lazy)
+    void* d_himg = nullptr;
+
+    // back-projection configuration
+    int bp_variant = 0;         // 0: 32x32 tile, R=8, WY=4;  1: 32x16, R=4, WY=4;  2: 32x16, R=8, WY=2
+    int bp_tw = 32, bp_th = 32, bp_r = 8, bp_threads = 128;
+    int bp_splits = 1, bp_chunk = 1, bp_seg = 0, bp_smem = 0;
+    fbp::BpParams bp{};
+
+    // filter configuration
+    int f_r = 9, f_threads = 0, f_smem = 0;
+    fbp::FilterParams fp{};
+
+    bool profiling = false;
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    bool ran_filter = false, ran_bp = false;
+
+    std::string err;
+};
+
+namespace {
+
+fbp_status fail(fbp_plan* p, fbp_status st, const std::string& msg)
+{
+    if (p) p->err = msg; else g_create_error = msg;
+    return st;
+}
+
+fbp_status cuda_fail(fbp_plan* p, cudaError_t e, const char* what)
+{
+    std::string m = std::string(what) + ": " + cudaGetErrorString(e);
+    cudaGetLastError();  // clear non-sticky error state
+    return fail(p, e == cudaErrorMemoryAllocation ? FBP_ENOMEM : FBP_ECUDA, m);
+}
+
+#define FBP_CUDA(plan, call)                                        \
+    do {                                                            \
+        cudaError_t e__ = (call);                                   \
+        if (e__ != cudaSuccess) return cuda_fail(plan, e__, #call); \
+    } while (0)
+
+// RAII device switch: the plan's device is made current for the call and restored after.
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; cudaGetLastError(); return; }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) { ok = false; cudaGetLastError(); }
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+int round_up(int v, int m) { return (v + m - 1) / m * m; }
+
+// ---- filter launch configuration -------------------------------------------------
+void configure_filter(fbp_plan* p)
+{
+    const int D = p->D;
+    const int de = (D + 1) / 2, dn = D / 2;
+    static const int cand[] = {5, 7, 9, 11, 13, 15};
+    int best_r = 9;
+    double best = -1.0;
+    const int forced = env_int("FBP_FILTER_R", 0);
+    for (int R : cand) {
+        const int w0 = (((de + R - 1) / R) + 31) / 32;
+        const int w1 = dn > 0 ? (((dn + R - 1) / R) + 31) / 32 : 0;
+        const double util = (double)D / ((double)R * 32.0 * (w0 + w1));
+        const double score = util * R / (R + 2.0);
+        if (forced == R) { best_r = R; break; }
+        if (score > best) { best = score; best_r = R; }
+    }
+    const int R = best_r;
+    p->f_r = R;
+    fbp::FilterParams& f = p->fp;
+    f.n_det = D;
+    f.de = de; f.dn = dn;
+    f.de_pad = round_up(de, R);
+    f.dn_pad = round_up(dn > 0 ? dn : 1, R);
+    f.wpr0 = (((de + R - 1) / R) + 31) / 32;
+    f.wpr1 = dn > 0 ? (((dn + R - 1) / R) + 31) / 32 : 0;
+    const int din_max = f.de_pad > f.dn_pad ? f.de_pad : f.dn_pad;
+    f.tab_off = din_max + 1;
+    f.tab_len = f.tab_off + de + R + 1;
+    f.y_pitch = round_up(D, 4);
+    const int wpr = f.wpr0 + f.wpr1;
+    const size_t row_bytes = (size_t)(f.de_pad + f.dn_pad + f.y_pitch) * p->esize;
+    const size_t tab_bytes = (size_t)round_up(f.tab_len, 4) * p->esize;
+    f.tab_len = round_up(f.tab_len, 4);
+    int rows = env_int("FBP_FILTER_ROWS", 0);
+    if (rows <= 0) {
+        rows = 8 / wpr;                       // aim at ~8 warps per CTA
+        const int by_grid = p->K / (2 * kNumSm);  // keep >= 2 CTAs per SM when K allows
+        if (rows > by_grid) rows = by_grid;
+    }
+    if (rows < 1) rows = 1;
+    while (rows > 1 && (rows * wpr * 32 > 512 || tab_bytes + rows * row_bytes > 100 * 1024)) --rows;
+    f.rows_per_cta = rows;
+    p->f_threads = rows * wpr * 32;
+    p->f_smem = (int)(tab_bytes + rows * row_bytes);
+}
+
+// ---- back-projection launch configuration ------------------------------------------
+void configure_bp(fbp_plan* p, const std::vector<double>& cs)
+{
+    p->bp_variant = env_int("FBP_BP_VARIANT", 0);
+    if (p->bp_variant < 0 || p->bp_variant > 2) p->bp_variant = 0;
+    switch (p->bp_variant) {
+        case 0: p->bp_th = 32; p->bp_r = 8; p->bp_threads = 128; break;
+        case 1: p->bp_th = 16; p->bp_r = 4; p->bp_threads = 128; break;
+        default: p->bp_th = 16; p->bp_r = 8; p->bp_threads = 64; break;
+    }
+    const int N = p->N, K = p->K;
+    const int tiles_x = (N + p->bp_tw - 1) / p->bp_tw;
+    const int tiles_y = (N + p->bp_th - 1) / p->bp_th;
+    double ext = 0.0;
+    for (int i = 0; i < K; ++i) {
+        const double e = (p->bp_tw - 1) * std::fabs(cs[2 * i]) + (p->bp_th - 1) * std::fabs(cs[2 * i + 1]);
+        if (e > ext) ext = e;
+    }
+    p->bp_seg = (int)std::ceil(ext) + 4;
+
+    // angle splits: fill 148 SMs evenly when one launch has few tiles
+    const long tiles = (long)tiles_x * tiles_y * p->max_batch;
+    int S = env_int("FBP_BP_SPLITS", 0);
+    if (S <= 0) {
+        const int s_max = K / 16 > 1 ? (K / 16 < 16 ? K / 16 : 16) : 1;
+        double best = -1.0;
+        S = 1;
+        for (int s = 1; s <= s_max; ++s) {
+            const long ctas = tiles * s;
+            const long waves = (ctas + kNumSm - 1) / kNumSm;
+            double eff = (double)ctas / (double)(waves * kNumSm);
+            if (ctas < 4L * kNumSm) eff *= 0.5 + 0.5 * (double)ctas / (4.0 * kNumSm);
+            eff -= 0.01 * (s - 1);  // splitting is not free: prefer fewer splits on ties
+            if (eff > best) { best = eff; S = s; }
+        }
+    }
+    if (S > K) S = K;
+    if (S < 1) S = 1;
+    p->bp_splits = S;
+    const int per = (K + S - 1) / S;
+
+    const size_t pair = 2 * p->esize, rec = 4 * p->esize;
+    const size_t per_angle = (size_t)p->bp_seg * pair + rec + sizeof(int);
+    int budget = env_int("FBP_BP_SMEM", 28 * 1024);
+    int chunk = env_int("FBP_BP_CHUNK", 0);
+    if (chunk <= 0) chunk = (int)(budget / per_angle);
+    if (chunk > per) chunk = per;
+    if (chunk < 1) chunk = 1;
+    p->bp_chunk = chunk;
+    p->bp_smem = (int)(per_angle * chunk + 16);
+
+    fbp::BpParams& b = p->bp;
+    b.n_angles = K; b.n_det = p->D; b.image_n = N;
+    b.tiles_x = tiles_x; b.tiles_y = tiles_y;
+    b.n_splits = S; b.chunk = chunk; b.seg_len = p->bp_seg;
+    b.c_n = 0.5 * (N - 1); b.c_d = 0.5 * (p->D - 1);
+    b.scale = kPi / K;
+}
+
+}  // namespace
+
+// ---- kernel launchers ---------------------------------------------------------------
+namespace {
+
+template <typename T, int R>
+cudaError_t launch_filter_r(const fbp_plan* p, const void* sino, void* filt, int batch, cudaStream_t st)
+{
+    fbp::FilterParams f = p->fp;
+    f.n_rows = batch * p->K;
+    const int grid = (f.n_rows + f.rows_per_cta - 1) / f.rows_per_cta;
+    auto kern = fbp::filter_kernel<T, R>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, p->f_smem);
+    if (e != cudaSuccess) return e;
+    kern<<<grid, p->f_threads, p->f_smem, st>>>(static_cast<const T*>(sino), static_cast<T*>(filt),
+                                                 static_cast<const T*>(p->d_taps), f, (T)(1.0 / p->d));
+    return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t launch_filter(const fbp_plan* p, const void* sino, void* filt, int batch, cudaStream_t st)
+{
+    switch (p->f_r) {
+        case 5: return launch_filter_r<T, 5>(p, sino, filt, batch, st);
+        case 7: return launch_filter_r<T, 7>(p, sino, filt, batch, st);
+        case 9: return launch_filter_r<T, 9>(p, sino, filt, batch, st);
+        case 11: return launch_filter_r<T, 11>(p, sino, filt, batch, st);
+        case 13: return launch_filter_r<T, 13>(p, sino, filt, batch, st);
+        default: return launch_filter_r<T, 15>(p, sino, filt, batch, st);
+    }
+}
+
+template <typename T, int R, int WY>
+cudaError_t launch_bp_v(const fbp_plan* p, const void* filt, void* out, int batch, cudaStream_t st)
+{
+    auto kern = fbp::backproject_kernel<T, R, WY>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, p->bp_smem);
+    if (e != cudaSuccess) return e;
+    dim3 grid(p->bp.tiles_x * p->bp.tiles_y, p->bp_splits, batch);
+    kern<<<grid, 32 * WY, p->bp_smem, st>>>(static_cast<const T*>(filt), static_cast<T*>(out), p->d_cs2,
+                                            p->bp, batch);
+    return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t launch_bp(const fbp_plan* p, const void* filt, void* image, int batch, cudaStream_t st)
+{
+    void* out = p->bp_splits > 1 ? p->d_part : image;
+    cudaError_t e;
+    switch (p->bp_variant) {
+        case 0: e = launch_bp_v<T, 8, 4>(p, filt, out, batch, st); break;
+        case 1: e = launch_bp_v<T, 4, 4>(p, filt, out, batch, st); break;
+        default: e = launch_bp_v<T, 8, 2>(p, filt, out, batch, st); break;
+    }
+    if (e != cudaSuccess || p->bp_splits == 1) return e;
+    const size_t n = (size_t)batch * p->N * p->N;
+    int blocks = (int)((n + 255) / 256);
+    if (blocks > kNumSm * 8) blocks = kNumSm * 8;
+    fbp::reduce_kernel<T><<<blocks, 256, 0, st>>>(static_cast<const T*>(p->d_part), static_cast<T*>(image), n,
+                                                 p->bp_splits, (T)p->bp.scale);
+    return cudaGetLastError();
+}
+
+bool aligned16(const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15u) == 0; }
+
+fbp_status check_call(fbp_plan* p, const void* a, const void* b, int batch)
+{
+    if (!p) return FBP_EINVAL;
+    if (!a || !b) return fail(p, FBP_EINVAL, "NULL device pointer");
+    if (!aligned16(a) || !aligned16(b)) return fail(p, FBP_EINVAL, "device pointers must be 16-byte aligned");
+    if (batch < 1 || batch > p->max_batch) return fail(p, FBP_EINVAL, "batch must be in [1, max_batch]");
+    return FBP_OK;
+}
+
+fbp_status run_filter(fbp_plan* p, const void* sino, void* filt, int batch, cudaStream_t st)
+{
+    if (p->profiling) FBP_CUDA(p, cudaEventRecord(p->ev[0], st));
+    cudaError_t e = p->dtype == FBP_F32 ? launch_filter<float>(p, sino, filt, batch, st)
+                                        : launch_filter<double>(p, sino, filt, batch, st);
+    if (e != cudaSuccess) return cuda_fail(p, e, "filter launch");
+    if (p->profiling) FBP_CUDA(p, cudaEventRecord(p->ev[1], st));
+    p->ran_filter = true;
+    return FBP_OK;
+}
+
+fbp_status run_bp(fbp_plan* p, const void* filt, void* image, int batch, cudaStream_t st)
+{
+    if (p->profiling) FBP_CUDA(p, cudaEventRecord(p->ev[2], st));
+    cudaError_t e = p->dtype == FBP_F32 ? launch_bp<float>(p, filt, image, batch, st)
+                                        : launch_bp<double>(p, filt, image, batch, st);
+    if (e != cudaSuccess) return cuda_fail(p, e, "back-projection launch");
+    if (p->profiling) FBP_CUDA(p, cudaEventRecord(p->ev[3], st));
+    p->ran_bp = true;
+    return FBP_OK;
+}
+
+}  // namespace
+
+// ---- C ABI ----------------------------------------------------------------------------
+extern "C" {
+
+fbp_status fbp_create(fbp_plan** out, int n_angles, int n_det, const double* angles_rad,
+                      double det_spacing, int image_n, double pixel_size, fbp_dtype dtype,
+                      int max_batch, int device)
+{
+    if (!out) return fail(nullptr, FBP_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!angles_rad) return fail(nullptr, FBP_EINVAL, "angles_rad is NULL");
+    if (n_angles < 1 || n_angles > (1 << 20)) return fail(nullptr, FBP_EINVAL, "n_angles must be in [1, 2^20]");
+    if (n_det < 2 || n_det > (1 << 20)) return fail(nullptr, FBP_EINVAL, "n_det must be in [2, 2^20]");
+    if (image_n < 1 || image_n > (1 << 16)) return fail(nullptr, FBP_EINVAL, "image_n must be in [1, 65536]");
+    if (!(det_spacing > 0.0) || !std::isfinite(det_spacing)) return fail(nullptr, FBP_EINVAL, "det_spacing must be finite and > 0");
+    if (!std::isfinite(pixel_size)) return fail(nullptr, FBP_EINVAL, "pixel_size must be finite");
+    if (dtype != FBP_F32 && dtype != FBP_F64) return fail(nullptr, FBP_EINVAL, "unknown dtype");
+    if (max_batch < 1 || max_batch > 65535) return fail(nullptr, FBP_EINVAL, "max_batch must be in [1, 65535]");
+    for (int i = 0; i < n_angles; ++i)
+        if (!std::isfinite(angles_rad[i])) return fail(nullptr, FBP_EINVAL, "non-finite angle");
+    const double pix = pixel_size > 0.0 ? pixel_size : det_spacing;
+
+    int ndev = 0;
+    cudaError_t ce = cudaGetDeviceCount(&ndev);
+    if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "cudaGetDeviceCount");
+    if (device < 0) {
+        ce = cudaGetDevice(&device);
+        if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "cudaGetDevice");
+    }
+    if (device >= ndev) return fail(nullptr, FBP_EINVAL, "no such CUDA device");
+    cudaDeviceProp prop;
+    ce = cudaGetDeviceProperties(&prop, device);
+    if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "cudaGetDeviceProperties");
+    if (prop.major != 10)
+        return fail(nullptr, FBP_EUNSUPPORTED, "libfbp is built for sm_100a (B200) only; no fallback path");
+
+    fbp_plan* p = new (std::nothrow) fbp_plan();
+    if (!p) return fail(nullptr, FBP_ENOMEM, "host allocation failed");
+    p->dtype = dtype; p->K = n_angles; p->D = n_det; p->N = image_n; p->max_batch = max_batch;
+    p->device = device; p->d = det_spacing; p->pix = pix;
+    p->esize = dtype == FBP_F32 ? 4 : 8;
+
+    // host tables in fp64: (cos, sin) * pix/d  (A0 of SURVEY.md 8(a))
+    std::vector<double> cs(2 * (size_t)n_angles);
+    const double ratio = pix / det_spacing;
+    for (int i = 0; i < n_angles; ++i) {
+        cs[2 * i] = std::cos(angles_rad[i]) * ratio;
+        cs[2 * i + 1] = std::sin(angles_rad[i]) * ratio;
+    }
+    configure_filter(p);
+    configure_bp(p, cs);
+
+    auto bail = [&](fbp_status st) { std::string m = p->err; fbp_destroy(p); g_create_error = m; return st; };
+    if (p->f_threads > 512) { p->err = "n_det too large for the row filter (more than 512 threads per row)"; return bail(FBP_EUNSUPPORTED); }
+    if (p->f_smem > 220 * 1024) { p->err = "n_det too large for the shared-memory row filter"; return bail(FBP_EUNSUPPORTED); }
+    if (p->bp_smem > 220 * 1024) { p->err = "pixel_size/det_spacing too large for the staged segment"; return bail(FBP_EUNSUPPORTED); }
+
+    DeviceGuard guard(device);
+    if (!guard.ok) { p->err = "cudaSetDevice failed"; return bail(FBP_ECUDA); }
+
+    // taps g[q] = h[2q+1] = -1/(pi^2 (2q+1)^2), index = q + tab_off, rounded once to dtype
+    const int tl = p->fp.tab_len;
+    std::vector<double> g64(tl);
+    for (int i = 0; i < tl; ++i) {
+        const double m = 2.0 * (double)(i - p->fp.tab_off) + 1.0;
+        g64[i] = -1.0 / (kPi * kPi * m * m);
+    }
+    std::vector<float> g32;
+    const void* gsrc = g64.data();
+    if (dtype == FBP_F32) { g32.assign(g64.begin(), g64.end()); gsrc = g32.data(); }
+
+#define FBP_TRY(call)                                                            \
+    do {                                                                         \
+        cudaError_t e__ = (call);                                                \
+        if (e__ != cudaSuccess) return bail(cuda_fail(p, e__, #call));           \
+    } while (0)
+    FBP_TRY(cudaMalloc(&p->d_cs2, sizeof(double2) * (size_t)n_angles));
+    FBP_TRY(cudaMemcpy(p->d_cs2, cs.data(), sizeof(double2) * (size_t)n_angles, cudaMemcpyHostToDevice));
+    FBP_TRY(cudaMalloc(&p->d_taps, p->esize * (size_t)tl));
+    FBP_TRY(cudaMemcpy(p->d_taps, gsrc, p->esize * (size_t)tl, cudaMemcpyHostToDevice));
+    FBP_TRY(cudaMalloc(&p->d_qwork, p->esize * (size_t)max_batch * n_angles * n_det));
+    if (p->bp_splits > 1)
+        FBP_TRY(cudaMalloc(&p->d_part, p->esize * (size_t)p->bp_splits * max_batch * image_n * image_n));
+    for (int i = 0; i < 4; ++i) FBP_TRY(cudaEventCreate(&p->ev[i]));
+#undef FBP_TRY
+    *out = p;
+    return FBP_OK;
+}
+
+void fbp_destroy(fbp_plan* p)
+{
+    if (!p) return;
+    {
+        DeviceGuard guard(p->device);
+        cudaFree(p->d_cs2); cudaFree(p->d_taps); cudaFree(p->d_qwork); cudaFree(p->d_part);
+        cudaFree(p->d_hsino); cudaFree(p->d_himg);
+        for (int i = 0; i < 4; ++i) if (p->ev[i]) cudaEventDestroy(p->ev[i]);
+        cudaGetLastError();
+    }
+    delete p;
+}
+
+const char* fbp_last_error(const fbp_plan* p) { return p ? p->err.c_str() : g_create_error.c_str(); }
+
+}  // extern "C"
+
+extern "C" {
+
+fbp_status fbp_filter(fbp_plan* p, const void* d_sino, void* d_filtered, int batch, void* stream)
+{
+    fbp_status st = check_call(p, d_sino, d_filtered, batch);
+    if (st != FBP_OK) return st;
+    if (d_sino == d_filtered) return fail(p, FBP_EINVAL, "fbp_filter: input and output may not alias");
+    DeviceGuard guard(p->device);
+    p->ran_filter = p->ran_bp = false;
+    return run_filter(p, d_sino, d_filtered, batch, static_cast<cudaStream_t>(stream));
+}
+
+fbp_status fbp_backproject(fbp_plan* p, const void* d_filtered, void* d_image, int batch, void* stream)
+{
+    fbp_status st = check_call(p, d_filtered, d_image, batch);
+    if (st != FBP_OK) return st;
+    DeviceGuard guard(p->device);
+    p->ran_filter = p->ran_bp = false;
+    return run_bp(p, d_filtered, d_image, batch, static_cast<cudaStream_t>(stream));
+}
+
+fbp_status fbp_reconstruct(fbp_plan* p, const void* d_sino, void* d_image, int batch, void* stream)
+{
+    fbp_status st = check_call(p, d_sino, d_image, batch);
+    if (st != FBP_OK) return st;
+    DeviceGuard guard(p->device);
+    p->ran_filter = p->ran_bp = false;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    st = run_filter(p, d_sino, p->d_qwork, batch, s);
+    if (st != FBP_OK) return st;
+    return run_bp(p, p->d_qwork, d_image, batch, s);
+}
+
+fbp_status fbp_reconstruct_host(fbp_plan* p, const void* h_sino, void* h_image, int batch, void* stream)
+{
+    if (!p) return FBP_EINVAL;
+    if (!h_sino || !h_image) return fail(p, FBP_EINVAL, "NULL host pointer");
+    if (batch < 1 || batch > p->max_batch) return fail(p, FBP_EINVAL, "batch must be in [1, max_batch]");
+    DeviceGuard guard(p->device);
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const size_t sino_bytes = p->esize * (size_t)p->K * p->D, img_bytes = p->esize * (size_t)p->N * p->N;
+    if (!p->d_hsino) FBP_CUDA(p, cudaMalloc(&p->d_hsino, sino_bytes * p->max_batch));
+    if (!p->d_himg) FBP_CUDA(p, cudaMalloc(&p->d_himg, img_bytes * p->max_batch));
+    FBP_CUDA(p, cudaMemcpyAsync(p->d_hsino, h_sino, sino_bytes * batch, cudaMemcpyHostToDevice, s));
+    p->ran_filter = p->ran_bp = false;
+    fbp_status st = run_filter(p, p->d_hsino, p->d_qwork, batch, s);
+    if (st != FBP_OK) return st;
+    st = run_bp(p, p->d_qwork, p->d_himg, batch, s);
+    if (st != FBP_OK) return st;
+    FBP_CUDA(p, cudaMemcpyAsync(h_image, p->d_himg, img_bytes * batch, cudaMemcpyDeviceToHost, s));
+    FBP_CUDA(p, cudaStreamSynchronize(s));
+    return FBP_OK;
+}
+
+int fbp_plan_info(const fbp_plan* p, int* out, int n)
+{
+    if (!p) return 0;
+    const int v[14] = {p->bp_tw, p->bp_th, p->bp_r, p->bp_splits, p->bp_chunk, p->bp_seg,
+                       p->bp.tiles_x * p->bp.tiles_y * p->bp_splits, p->bp_threads, p->bp_smem,
+                       p->f_r, p->f_threads, p->fp.rows_per_cta, p->f_smem,
+                       p->bp_splits > 1 ? 3 : 2};
+    if (out) for (int i = 0; i < n && i < 14; ++i) out[i] = v[i];
+    return 14;
+}
+
+fbp_status fbp_set_profiling(fbp_plan* p, int enable)
+{
+    if (!p) return FBP_EINVAL;
+    p->profiling = enable != 0;
+    p->ran_filter = p->ran_bp = false;
+    return FBP_OK;
+}
+
+fbp_status fbp_get_kernel_ms(fbp_plan* p, float* filter_ms, float* backproject_ms)
+{
+    if (!p) return FBP_EINVAL;
+    if (!p->profiling) return fail(p, FBP_EINVAL, "profiling is off (fbp_set_profiling)");
+    DeviceGuard guard(p->device);
+    float f = 0.f, b = 0.f;
+    if (p->ran_filter) {
+        FBP_CUDA(p, cudaEventSynchronize(p->ev[1]));
+        FBP_CUDA(p, cudaEventElapsedTime(&f, p->ev[0], p->ev[1]));
+    }
+    if (p->ran_bp) {
+        FBP_CUDA(p, cudaEventSynchronize(p->ev[3]));
+        FBP_CUDA(p, cudaEventElapsedTime(&b, p->ev[2], p->ev[3]));
+    }
+    if (filter_ms) *filter_ms = f;
+    if (backproject_ms) *backproject_ms = b;
+    return FBP_OK;
+}
+
+}  // extern "C"

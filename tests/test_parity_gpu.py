@@ -1,0 +1,274 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU fp64 oracle, element by
+element on the same seeded inputs.  Tolerances are BASELINE.json's:
+  fp64: max|f_gpu - f_oracle| / max|f_oracle| <= 1e-12
+  fp32: max-abs <= 1e-4 * DR and RMSE <= 1e-5 * DR,  DR = max(f_oracle) - min(f_oracle)
+fp32 inputs are rounded to fp32 once and the oracle consumes those rounded values.
+The filter alone is held to 1e-12 (fp64) and 1e-5 (fp32; a
+~D/2-term fp32 sum) of max|Q_oracle|."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from paper_2109_02174_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+F64_TOL = 1e-12
+F32_MAXABS, F32_RMSE = 1e-4, 1e-5
+F32_FILTER_TOL = 1e-5
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _np_dtype(dt):
+    return np.float32 if dt == "f32" else np.float64
+
+
+def _to_dev(a, dt):
+    torch = _torch()
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=_np_dtype(dt))).cuda()
+
+
+def check_image(gpu, ref, dt, what=""):
+    gpu = np.asarray(gpu, dtype=np.float64)
+    ref = np.asarray(ref, dtype=np.float64)
+    assert gpu.shape == ref.shape
+    err = np.abs(gpu - ref)
+    if dt == "f64":
+        rel = err.max() / max(np.abs(ref).max(), 1e-300)
+        assert rel <= F64_TOL, "%s fp64 rel max-abs %.3e" % (what, rel)
+        return rel
+    dr = max(ref.max() - ref.min(), 1e-30)
+    mx, rmse = err.max() / dr, math.sqrt(float(np.mean(err * err))) / dr
+    assert mx <= F32_MAXABS, "%s fp32 max-abs/DR %.3e" % (what, mx)
+    assert rmse <= F32_RMSE, "%s fp32 RMSE/DR %.3e" % (what, rmse)
+    return mx
+
+
+def check_filter(gpu, ref, dt, what=""):
+    gpu = np.asarray(gpu, dtype=np.float64)
+    rel = np.abs(gpu - ref).max() / max(np.abs(ref).max(), 1e-300)
+    assert rel <= (F64_TOL if dt == "f64" else F32_FILTER_TOL), "%s filter rel %.3e" % (what, rel)
+    return rel
+
+
+def run_case(fbp, oracle, sino64, angles, n, dt, d=1.0, pix=None, what=""):
+    """Full three-way check of one geometry: filter, back-projection, reconstruct."""
+    torch = _torch()
+    sino64 = np.asarray(sino64, dtype=np.float64)
+    if sino64.ndim == 2:
+        sino64 = sino64[None]
+    b, k, dd = sino64.shape
+    sino_in = sino64.astype(_np_dtype(dt))          # rounded once
+    sino_ref = sino_in.astype(np.float64)
+    plan = fbp.Plan(list(angles), dd, n, det_spacing=d, pixel_size=0.0 if pix is None else pix, dtype=dt, max_batch=b)
+    try:
+        ds = _to_dev(sino_in, dt)
+        q_gpu = plan.filter(ds)
+        q_ref = oracle.filter_sinogram(sino_ref, d)
+        check_filter(q_gpu.cpu().numpy(), q_ref, dt, what)
+        # back-projection alone, fed the oracle's Q rounded to the dtype
+        q_in = q_ref.astype(_np_dtype(dt))
+        f_ref_bp = oracle.backproject(q_in.astype(np.float64), angles, n, d, pix)
+        f_bp = plan.backproject(_to_dev(q_in, dt))
+        check_image(f_bp.cpu().numpy(), f_ref_bp, dt, what + " bp")
+        # whole chain
+        f_ref = oracle.reconstruct(sino_ref, angles, n, d, pix)
+        f_gpu = plan.reconstruct(ds)
+        worst = check_image(f_gpu.cpu().numpy(), f_ref, dt, what + " recon")
+        # reconstruct == backproject(filter) bit for bit (include/fbp.h)
+        f_two = plan.backproject(q_gpu)
+        torch.cuda.synchronize()
+        assert torch.equal(f_two, f_gpu)
+        return worst
+    finally:
+        plan.close()
+
+
+@pytest.mark.parametrize("cfg_id,dt", [(1, "f32"), (2, "f32"), (3, "f32"), (3, "f64"), (1, "f64")])
+def test_configs_full_images(fbp, oracle, cfg_id, dt):
+    cfg = I.CONFIGS[cfg_id]
+    run_case(fbp, oracle, I.config_sinogram(cfg_id), I.config_angles(cfg_id), cfg.image_n, dt, what=cfg.name)
+
+
+ODD_CASES = [
+    # (N, K, D, d, pix, angle kind)
+    (1, 1, 2, 1.0, None, "uniform"),
+    (7, 1, 11, 1.0, None, "uniform"),
+    (33, 5, 48, 1.0, None, "uniform"),          # N odd, D even, ragged tiles
+    (65, 37, 93, 0.5, 0.5, "uniform"),
+    (40, 23, 70, 2.0, 1.0, "random"),           # d != pixel, non-uniform angles
+    (50, 16, 40, 1.0, 1.0, "full"),             # detector too short: rays miss it; angles over 2 pi
+    (96, 64, 150, 0.7, 1.3, "random"),          # pixel > d: long segments, bank conflicts allowed
+    (130, 31, 185, 1.0, None, "uniform"),       # several tiles + ragged tail
+]
+
+
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+@pytest.mark.parametrize("case", ODD_CASES)
+def test_odd_shapes_random_sinograms(fbp, oracle, case, dt):
+    n, k, dd, d, pix, kind = case
+    rng = np.random.default_rng(1000 + n + k)
+    if kind == "uniform":
+        ang = I.uniform_angles(k)
+    elif kind == "full":
+        ang = I.uniform_angles(k, 2 * math.pi)
+    else:
+        ang = np.sort(rng.uniform(-1.0, 4.0, size=k))
+    sino = I.random_sinogram(77 + n, 3, k, dd)
+    run_case(fbp, oracle, sino, ang, n, dt, d, pix, what="odd%s" % (case,))
+
+
+def _sample_pixels(n, count, seed):
+    rng = np.random.default_rng(seed)
+    rows = rng.integers(0, n, size=count)
+    cols = rng.integers(0, n, size=count)
+    # always include the corners, the centre and tile-boundary pixels
+    extra = [(0, 0), (0, n - 1), (n - 1, 0), (n - 1, n - 1), (n // 2, n // 2), (31, 32), (32, 31), (n - 33, n - 32)]
+    rows = np.concatenate([rows, [e[0] for e in extra]]).astype(np.int32)
+    cols = np.concatenate([cols, [e[1] for e in extra]]).astype(np.int32)
+    return rows, cols
+
+
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+def test_cfg5_full_size_sampled(fbp, oracle, dt):
+    """2048^2 x 1800 x 2897 in the launch configuration bench.py uses; the oracle checks
+    sampled filter rows and sampled pixels one by one."""
+    cfg = I.CONFIGS[5]
+    ang = I.config_angles(5)
+    sino_in = I.config_slice(5).astype(_np_dtype(dt))
+    sino_ref = sino_in.astype(np.float64)
+    plan = fbp.Plan(list(ang), cfg.n_det, cfg.image_n, dtype=dt, max_batch=1)
+    try:
+        ds = _to_dev(sino_in, dt)
+        q_gpu = plan.filter(ds).cpu().numpy()
+        rows_f = np.array([0, 1, 449, 900, 1234, 1799], dtype=np.int32)
+        q_rows = oracle.filter_rows(sino_ref, rows_f)
+        check_filter(q_gpu[rows_f], q_rows, dt, "cfg5")
+        # whole chain on sampled pixels: the oracle filters the full sinogram itself (nothing
+        # the CUDA path produced is ever an oracle input) and back-projects the samples; DR
+        # is taken over the oracle's samples.
+        f_gpu = plan.reconstruct(ds).cpu().numpy()
+        rr, cc = _sample_pixels(cfg.image_n, 3000, 55)
+        q_ref = oracle.filter_sinogram(sino_ref)
+        check_filter(q_gpu, q_ref, dt, "cfg5 all rows")
+        f_ref = oracle.backproject_pixels(q_ref, ang, cfg.image_n, rr, cc)
+        check_image(f_gpu[rr, cc], f_ref, dt, "cfg5 sampled")
+    finally:
+        plan.close()
+
+
+def test_cfg4_batch_sampled(fbp, oracle):
+    """64 slices x 512^2 x 720 in one launch; three slices checked on sampled pixels, one in full."""
+    cfg = I.CONFIGS[4]
+    ang = I.config_angles(4)
+    sino_in = I.config_sinogram(4).astype(np.float32)
+    plan = fbp.Plan(list(ang), cfg.n_det, cfg.image_n, dtype="f32", max_batch=cfg.batch)
+    try:
+        ds = _to_dev(sino_in, "f32")
+        q_gpu = plan.filter(ds).cpu().numpy()
+        f_gpu = plan.reconstruct(ds).cpu().numpy()
+        for s in (0, 37, 63):
+            q_ref = oracle.filter_sinogram(sino_in[s].astype(np.float64))
+            check_filter(q_gpu[s], q_ref, "f32", "cfg4 s%d" % s)
+            rr, cc = _sample_pixels(cfg.image_n, 2000, 400 + s)
+            f_ref = oracle.backproject_pixels(q_ref, ang, cfg.image_n, rr, cc)
+            check_image(f_gpu[s][rr, cc], f_ref, "f32", "cfg4 s%d" % s)
+        f_full = oracle.reconstruct(sino_in[5].astype(np.float64), ang, cfg.image_n)
+        check_image(f_gpu[5], f_full, "f32", "cfg4 s5 full")
+    finally:
+        plan.close()
+
+
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+def test_bit_identical_across_runs(fbp, dt):
+    """PAPER.md:218 reports run-to-run noise for its parallel versions; here 10 runs are memcmp-equal,
+    also with other work interleaved on the device."""
+    torch = _torch()
+    cfg = I.CONFIGS[3]
+    ds = _to_dev(I.config_sinogram(3), dt)
+    plan = fbp.Plan(list(I.config_angles(3)), cfg.n_det, cfg.image_n, dtype=dt)
+    try:
+        first = plan.reconstruct(ds).clone()
+        junk = torch.randn(4096, 4096, device="cuda")
+        for it in range(10):
+            if it % 2:
+                junk = junk @ junk.t() * 1e-4
+            out = plan.reconstruct(ds)
+            torch.cuda.synchronize()
+            assert torch.equal(out, first)
+    finally:
+        plan.close()
+
+
+@pytest.mark.parametrize("splits", [1, 2, 5, 7])
+@pytest.mark.parametrize("variant", [0, 1, 2])
+def test_angle_splits_and_tile_variants(fbp, oracle, splits, variant, monkeypatch):
+    monkeypatch.setenv("FBP_BP_SPLITS", str(splits))
+    monkeypatch.setenv("FBP_BP_VARIANT", str(variant))
+    monkeypatch.setenv("FBP_BP_CHUNK", "13")
+    n, k, dd = 100, 45, 150
+    ang = I.uniform_angles(k)
+    for dt in ("f32", "f64"):
+        q = I.random_sinogram(9, 2, k, dd).astype(_np_dtype(dt))
+        plan = fbp.Plan(list(ang), dd, n, dtype=dt, max_batch=2)
+        try:
+            assert plan.info()["bp_angle_splits"] == splits
+            f = plan.backproject(_to_dev(q, dt)).cpu().numpy()
+            check_image(f, oracle.backproject(q.astype(np.float64), ang, n), dt, "split%d v%d" % (splits, variant))
+        finally:
+            plan.close()
+
+
+def test_host_path_matches_device_path(fbp):
+    torch = _torch()
+    cfg = I.CONFIGS[2]
+    sino = torch.from_numpy(I.config_sinogram(2).astype(np.float32)).pin_memory()
+    plan = fbp.Plan(list(I.config_angles(2)), cfg.n_det, cfg.image_n, dtype="f32")
+    try:
+        dev = plan.reconstruct(sino.cuda())
+        host = torch.empty((1, cfg.image_n, cfg.image_n), dtype=torch.float32).pin_memory()
+        fbp.fbp_reconstruct_host(plan.handle, sino, host, 1)
+        assert torch.equal(dev.cpu(), host)
+    finally:
+        plan.close()
+
+
+def test_error_paths_on_device(fbp):
+    torch = _torch()
+    plan = fbp.Plan(list(I.uniform_angles(8)), 16, 8, dtype="f32", max_batch=2)
+    try:
+        s = torch.zeros(3, 8, 16, device="cuda")
+        img = torch.full((3, 8, 8), 7.0, device="cuda")
+        for bad_batch in (0, 3):
+            with pytest.raises(fbp.FbpError) as ei:
+                fbp.fbp_reconstruct(plan.handle, s, img, bad_batch)
+            assert ei.value.status == fbp.FBP_EINVAL
+        with pytest.raises(fbp.FbpError):
+            fbp.fbp_reconstruct(plan.handle, s.data_ptr() + 4, img, 1)   # misaligned
+        with pytest.raises(fbp.FbpError):
+            fbp.fbp_filter(plan.handle, s, s, 1)                          # aliasing
+        with pytest.raises(fbp.FbpError):
+            fbp.fbp_backproject(plan.handle, 0, img, 1)                   # NULL
+        torch.cuda.synchronize()
+        assert bool((img == 7.0).all())                                   # outputs untouched
+        assert fbp.fbp_last_error(plan.handle) != ""
+    finally:
+        plan.close()
+
+
+def test_profiling_hooks(fbp):
+    cfg = I.CONFIGS[1]
+    plan = fbp.Plan(list(I.config_angles(1)), cfg.n_det, cfg.image_n, dtype="f32")
+    try:
+        fbp.fbp_set_profiling(plan.handle, True)
+        plan.reconstruct(_to_dev(I.config_sinogram(1), "f32"))
+        f_ms, b_ms = fbp.fbp_get_kernel_ms(plan.handle)
+        assert f_ms > 0 and b_ms > 0
+    finally:
+        plan.close()
