@@ -23,7 +23,7 @@ EXPORTS = (
 PLAN_INFO_FIELDS = (
     "bp_tile_w", "bp_tile_h", "bp_pixels_per_thread", "bp_angle_splits", "bp_angles_per_chunk",
     "bp_segment_len", "bp_ctas_per_slice", "bp_threads", "bp_smem_bytes",
-    "filter_outputs_per_thread", "filter_threads", "filter_rows_per_cta", "filter_smem_bytes",
+    "filter_outputs_per_thread", "filter_threads", "filter_input_slices", "filter_smem_bytes",
     "kernels_per_reconstruct",
 )
 

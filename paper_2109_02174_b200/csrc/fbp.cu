@@ -5,6 +5,7 @@
 
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
@@ -41,8 +42,9 @@ struct fbp_plan {
 
     // device tables / scratch
     double2* d_cs2 = nullptr;   // [K] (cos, sin) * pix/d, fp64
-    void* d_taps = nullptr;     // [tab_len] dtype
-    void* d_qwork = nullptr;    // [max_batch][K][D] filtered sinogram (fbp_reconstruct)
+    void* d_taps = nullptr;     // [tab_len] dtype: G[q + tab_off] = g[q]
+    void* d_rho = nullptr;      // [D] dtype: conditioning term of the filter (fbp_filter.cuh)
+    void* d_ent = nullptr;      // [max_batch][K][ent_pitch] BpEntry: back-projector operands
     void* d_part = nullptr;     // [S][max_batch][N][N] partial images when S > 1
     void* d_hsino = nullptr;    // host-path staging (lazy)
     void* d_himg = nullptr;
@@ -54,7 +56,7 @@ struct fbp_plan {
     fbp::BpParams bp{};
 
     // filter configuration
-    int f_r = 9, f_threads = 0, f_smem = 0;
+    int f_r = 9, f_threads = 0, f_smem = 0, f_tab_len = 0;
     fbp::FilterParams fp{};
 
     bool profiling = false;
@@ -100,6 +102,7 @@ struct DeviceGuard {
 int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
 // ---- filter launch configuration -------------------------------------------------
+// One CTA per row; warps = 2 parities x n_ob output blocks (32*R outputs) x n_sb input slices.
 void configure_filter(fbp_plan* p)
 {
     const int D = p->D;
@@ -109,10 +112,9 @@ void configure_filter(fbp_plan* p)
     double best = -1.0;
     const int forced = env_int("FBP_FILTER_R", 0);
     for (int R : cand) {
-        const int w0 = (((de + R - 1) / R) + 31) / 32;
-        const int w1 = dn > 0 ? (((dn + R - 1) / R) + 31) / 32 : 0;
-        const double util = (double)D / ((double)R * 32.0 * (w0 + w1));
-        const double score = util * R / (R + 2.0);
+        const int n_ob = (de + 32 * R - 1) / (32 * R);
+        const double util = (double)de / ((double)n_ob * 32 * R);
+        const double score = util * R / (R + 3.0);
         if (forced == R) { best_r = R; break; }
         if (score > best) { best = score; best_r = R; }
     }
@@ -121,29 +123,27 @@ void configure_filter(fbp_plan* p)
     fbp::FilterParams& f = p->fp;
     f.n_det = D;
     f.de = de; f.dn = dn;
-    f.de_pad = round_up(de, R);
-    f.dn_pad = round_up(dn > 0 ? dn : 1, R);
-    f.wpr0 = (((de + R - 1) / R) + 31) / 32;
-    f.wpr1 = dn > 0 ? (((dn + R - 1) / R) + 31) / 32 : 0;
+    f.n_ob = (de + 32 * R - 1) / (32 * R);
+    // input slices: enough warps to fill 148 SMs with ~16 warps each, at most 16 warps per CTA
+    int sb = env_int("FBP_FILTER_SB", 0);
+    if (sb <= 0) {
+        sb = (int)std::ceil(16.0 * kNumSm / ((double)p->K * 2 * f.n_ob));
+        if (sb < 2) sb = 2;
+        if (sb > 8) sb = 8;
+    }
+    while (sb > 1 && 2 * f.n_ob * sb > 16) --sb;
+    f.n_sb = sb;
+    f.de_pad = round_up(de, sb * R);
+    f.dn_pad = round_up(dn, sb * R);
     const int din_max = f.de_pad > f.dn_pad ? f.de_pad : f.dn_pad;
     f.tab_off = din_max + 1;
-    f.tab_len = f.tab_off + de + R + 1;
-    f.y_pitch = round_up(D, 4);
-    const int wpr = f.wpr0 + f.wpr1;
-    const size_t row_bytes = (size_t)(f.de_pad + f.dn_pad + f.y_pitch) * p->esize;
-    const size_t tab_bytes = (size_t)round_up(f.tab_len, 4) * p->esize;
-    f.tab_len = round_up(f.tab_len, 4);
-    int rows = env_int("FBP_FILTER_ROWS", 0);
-    if (rows <= 0) {
-        rows = 8 / wpr;                       // aim at ~8 warps per CTA
-        const int by_grid = p->K / (2 * kNumSm);  // keep >= 2 CTAs per SM when K allows
-        if (rows > by_grid) rows = by_grid;
-    }
-    if (rows < 1) rows = 1;
-    while (rows > 1 && (rows * wpr * 32 > 512 || tab_bytes + rows * row_bytes > 100 * 1024)) --rows;
-    f.rows_per_cta = rows;
-    p->f_threads = rows * wpr * 32;
-    p->f_smem = (int)(tab_bytes + rows * row_bytes);
+    f.tab_cnt = din_max + f.n_ob * 32 * R + R + 1;
+    p->f_tab_len = f.tab_off + f.tab_cnt + 2;
+    f.x_pitch = round_up(din_max, 4);
+    p->f_threads = 2 * f.n_ob * sb * 32;
+    const size_t words = 2 * (size_t)f.tab_cnt + 2 * (size_t)f.x_pitch + 2 * (size_t)f.n_ob * 32 +
+                         (size_t)(1 + sb) * 2 * f.n_ob * 32 * R;
+    p->f_smem = (int)(words * p->esize + 16);
 }
 
 // ---- back-projection launch configuration ------------------------------------------
@@ -158,7 +158,8 @@ void configure_bp(fbp_plan* p, const std::vector<double>& cs)
     }
     const int N = p->N, K = p->K;
     const int tiles_x = (N + p->bp_tw - 1) / p->bp_tw;
-    const int tiles_y = (N + p->bp_th - 1) / p->bp_th;
+    const int half_rows = (N + 1) / 2;  // primary (top) half; the mirror pixels come for free
+    const int tiles_y = (half_rows + p->bp_th - 1) / p->bp_th;
     double ext = 0.0;
     for (int i = 0; i < K; ++i) {
         const double e = (p->bp_tw - 1) * std::fabs(cs[2 * i]) + (p->bp_th - 1) * std::fabs(cs[2 * i + 1]);
@@ -187,20 +188,24 @@ void configure_bp(fbp_plan* p, const std::vector<double>& cs)
     p->bp_splits = S;
     const int per = (K + S - 1) / S;
 
-    const size_t pair = 2 * p->esize, rec = 4 * p->esize;
-    const size_t per_angle = (size_t)p->bp_seg * pair + rec + sizeof(int);
-    int budget = env_int("FBP_BP_SMEM", 28 * 1024);
+    const size_t entry = 4 * p->esize, rec = 4 * p->esize;
+    const size_t per_angle = (size_t)p->bp_seg * entry + rec;
+    int budget = env_int("FBP_BP_SMEM", 24 * 1024);
     int chunk = env_int("FBP_BP_CHUNK", 0);
     if (chunk <= 0) chunk = (int)(budget / per_angle);
     if (chunk > per) chunk = per;
     if (chunk < 1) chunk = 1;
     p->bp_chunk = chunk;
-    p->bp_smem = (int)(per_angle * chunk + 16);
+    p->bp_smem = (int)(per_angle * chunk + 16 + 128);
 
     fbp::BpParams& b = p->bp;
     b.n_angles = K; b.n_det = p->D; b.image_n = N;
     b.tiles_x = tiles_x; b.tiles_y = tiles_y;
     b.n_splits = S; b.chunk = chunk; b.seg_len = p->bp_seg;
+    b.half_rows = half_rows;
+    b.ent_guard = p->bp_seg + 1;                       // >= L+1 zero entries on both sides
+    b.ent_pitch = p->D + 2 * b.ent_guard;
+    p->fp.ent_guard = b.ent_guard; p->fp.ent_pitch = b.ent_pitch;
     b.c_n = 0.5 * (N - 1); b.c_d = 0.5 * (p->D - 1);
     b.scale = kPi / K;
 }
@@ -211,53 +216,65 @@ void configure_bp(fbp_plan* p, const std::vector<double>& cs)
 namespace {
 
 template <typename T, int R>
-cudaError_t launch_filter_r(const fbp_plan* p, const void* sino, void* filt, int batch, cudaStream_t st)
+cudaError_t launch_filter_r(const fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st)
 {
     fbp::FilterParams f = p->fp;
     f.n_rows = batch * p->K;
-    const int grid = (f.n_rows + f.rows_per_cta - 1) / f.rows_per_cta;
     auto kern = fbp::filter_kernel<T, R>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, p->f_smem);
     if (e != cudaSuccess) return e;
-    kern<<<grid, p->f_threads, p->f_smem, st>>>(static_cast<const T*>(sino), static_cast<T*>(filt),
-                                                 static_cast<const T*>(p->d_taps), f, (T)(1.0 / p->d));
+    kern<<<f.n_rows, p->f_threads, p->f_smem, st>>>(static_cast<const T*>(sino), static_cast<T*>(filt),
+                                                     static_cast<fbp::BpEntry<T>*>(ent),
+                                                     static_cast<const T*>(p->d_taps),
+                                                     static_cast<const T*>(p->d_rho), f, (T)(1.0 / p->d));
     return cudaGetLastError();
 }
 
+// filt and/or ent may be NULL: plain rows (fbp_filter) and/or interleaved entries (fbp_reconstruct)
 template <typename T>
-cudaError_t launch_filter(const fbp_plan* p, const void* sino, void* filt, int batch, cudaStream_t st)
+cudaError_t launch_filter(const fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st)
 {
     switch (p->f_r) {
-        case 5: return launch_filter_r<T, 5>(p, sino, filt, batch, st);
-        case 7: return launch_filter_r<T, 7>(p, sino, filt, batch, st);
-        case 9: return launch_filter_r<T, 9>(p, sino, filt, batch, st);
-        case 11: return launch_filter_r<T, 11>(p, sino, filt, batch, st);
-        case 13: return launch_filter_r<T, 13>(p, sino, filt, batch, st);
-        default: return launch_filter_r<T, 15>(p, sino, filt, batch, st);
+        case 5: return launch_filter_r<T, 5>(p, sino, filt, ent, batch, st);
+        case 7: return launch_filter_r<T, 7>(p, sino, filt, ent, batch, st);
+        case 9: return launch_filter_r<T, 9>(p, sino, filt, ent, batch, st);
+        case 11: return launch_filter_r<T, 11>(p, sino, filt, ent, batch, st);
+        case 13: return launch_filter_r<T, 13>(p, sino, filt, ent, batch, st);
+        default: return launch_filter_r<T, 15>(p, sino, filt, ent, batch, st);
     }
 }
 
+template <typename T>
+cudaError_t launch_entries(const fbp_plan* p, const void* filt, int batch, cudaStream_t st)
+{
+    fbp::entries_kernel<T><<<batch * p->K, 256, 0, st>>>(static_cast<const T*>(filt),
+                                                         static_cast<fbp::BpEntry<T>*>(p->d_ent), p->D,
+                                                         p->bp.ent_pitch, p->bp.ent_guard);
+    return cudaGetLastError();
+}
+
 template <typename T, int R, int WY>
-cudaError_t launch_bp_v(const fbp_plan* p, const void* filt, void* out, int batch, cudaStream_t st)
+cudaError_t launch_bp_v(const fbp_plan* p, void* out, int batch, cudaStream_t st)
 {
     auto kern = fbp::backproject_kernel<T, R, WY>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, p->bp_smem);
     if (e != cudaSuccess) return e;
     dim3 grid(p->bp.tiles_x * p->bp.tiles_y, p->bp_splits, batch);
-    kern<<<grid, 32 * WY, p->bp_smem, st>>>(static_cast<const T*>(filt), static_cast<T*>(out), p->d_cs2,
-                                            p->bp, batch);
+    kern<<<grid, 32 * WY, p->bp_smem, st>>>(static_cast<const fbp::BpEntry<T>*>(p->d_ent), static_cast<T*>(out),
+                                            p->d_cs2, p->bp, batch);
     return cudaGetLastError();
 }
 
+// back-projection of the plan's entry buffer into `image`
 template <typename T>
-cudaError_t launch_bp(const fbp_plan* p, const void* filt, void* image, int batch, cudaStream_t st)
+cudaError_t launch_bp(const fbp_plan* p, void* image, int batch, cudaStream_t st)
 {
     void* out = p->bp_splits > 1 ? p->d_part : image;
     cudaError_t e;
     switch (p->bp_variant) {
-        case 0: e = launch_bp_v<T, 8, 4>(p, filt, out, batch, st); break;
-        case 1: e = launch_bp_v<T, 4, 4>(p, filt, out, batch, st); break;
-        default: e = launch_bp_v<T, 8, 2>(p, filt, out, batch, st); break;
+        case 0: e = launch_bp_v<T, 8, 4>(p, out, batch, st); break;
+        case 1: e = launch_bp_v<T, 4, 4>(p, out, batch, st); break;
+        default: e = launch_bp_v<T, 8, 2>(p, out, batch, st); break;
     }
     if (e != cudaSuccess || p->bp_splits == 1) return e;
     const size_t n = (size_t)batch * p->N * p->N;
@@ -279,22 +296,28 @@ fbp_status check_call(fbp_plan* p, const void* a, const void* b, int batch)
     return FBP_OK;
 }
 
-fbp_status run_filter(fbp_plan* p, const void* sino, void* filt, int batch, cudaStream_t st)
+fbp_status run_filter(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st)
 {
     if (p->profiling) FBP_CUDA(p, cudaEventRecord(p->ev[0], st));
-    cudaError_t e = p->dtype == FBP_F32 ? launch_filter<float>(p, sino, filt, batch, st)
-                                        : launch_filter<double>(p, sino, filt, batch, st);
+    cudaError_t e = p->dtype == FBP_F32 ? launch_filter<float>(p, sino, filt, ent, batch, st)
+                                        : launch_filter<double>(p, sino, filt, ent, batch, st);
     if (e != cudaSuccess) return cuda_fail(p, e, "filter launch");
     if (p->profiling) FBP_CUDA(p, cudaEventRecord(p->ev[1], st));
     p->ran_filter = true;
     return FBP_OK;
 }
 
+// filt != NULL: convert plain filtered rows to entries first (fbp_backproject);
+// filt == NULL: the entry buffer was already written by the filter (fbp_reconstruct).
 fbp_status run_bp(fbp_plan* p, const void* filt, void* image, int batch, cudaStream_t st)
 {
+    cudaError_t e = cudaSuccess;
+    if (filt) {
+        e = p->dtype == FBP_F32 ? launch_entries<float>(p, filt, batch, st) : launch_entries<double>(p, filt, batch, st);
+        if (e != cudaSuccess) return cuda_fail(p, e, "entries launch");
+    }
     if (p->profiling) FBP_CUDA(p, cudaEventRecord(p->ev[2], st));
-    cudaError_t e = p->dtype == FBP_F32 ? launch_bp<float>(p, filt, image, batch, st)
-                                        : launch_bp<double>(p, filt, image, batch, st);
+    e = p->dtype == FBP_F32 ? launch_bp<float>(p, image, batch, st) : launch_bp<double>(p, image, batch, st);
     if (e != cudaSuccess) return cuda_fail(p, e, "back-projection launch");
     if (p->profiling) FBP_CUDA(p, cudaEventRecord(p->ev[3], st));
     p->ran_bp = true;
@@ -363,15 +386,35 @@ fbp_status fbp_create(fbp_plan** out, int n_angles, int n_det, const double* ang
     if (!guard.ok) { p->err = "cudaSetDevice failed"; return bail(FBP_ECUDA); }
 
     // taps g[q] = h[2q+1] = -1/(pi^2 (2q+1)^2), index = q + tab_off, rounded once to dtype
-    const int tl = p->fp.tab_len;
+    const int tl = p->f_tab_len;
     std::vector<double> g64(tl);
     for (int i = 0; i < tl; ++i) {
         const double m = 2.0 * (double)(i - p->fp.tab_off) + 1.0;
         g64[i] = -1.0 / (kPi * kPi * m * m);
     }
-    std::vector<float> g32;
+    // conditioning term rho[n] = 1/4 + sum_{b=0}^{din_pad(p)-1} g[a - b - (1-p)], n = 2a + p:
+    // what filtering a constant row (padding included) gives; fp64, smallest terms first
+    std::vector<double> rho64(n_det);
+    for (int n = 0; n < n_det; ++n) {
+        const int par = n & 1, a = n >> 1;
+        const int din_pad = par ? p->fp.de_pad : p->fp.dn_pad;
+        std::vector<double> terms(din_pad);
+        for (int b = 0; b < din_pad; ++b) {
+            const double m = 2.0 * (double)(a - b - (1 - par)) + 1.0;
+            terms[b] = 1.0 / (kPi * kPi * m * m);
+        }
+        std::sort(terms.begin(), terms.end());
+        double ssum = 0.0;
+        for (double t : terms) ssum += t;
+        rho64[n] = 0.25 - ssum;
+    }
+    std::vector<float> g32, rho32;
     const void* gsrc = g64.data();
-    if (dtype == FBP_F32) { g32.assign(g64.begin(), g64.end()); gsrc = g32.data(); }
+    const void* rsrc = rho64.data();
+    if (dtype == FBP_F32) {
+        g32.assign(g64.begin(), g64.end()); gsrc = g32.data();
+        rho32.assign(rho64.begin(), rho64.end()); rsrc = rho32.data();
+    }
 
 #define FBP_TRY(call)                                                            \
     do {                                                                         \
@@ -382,7 +425,9 @@ fbp_status fbp_create(fbp_plan** out, int n_angles, int n_det, const double* ang
     FBP_TRY(cudaMemcpy(p->d_cs2, cs.data(), sizeof(double2) * (size_t)n_angles, cudaMemcpyHostToDevice));
     FBP_TRY(cudaMalloc(&p->d_taps, p->esize * (size_t)tl));
     FBP_TRY(cudaMemcpy(p->d_taps, gsrc, p->esize * (size_t)tl, cudaMemcpyHostToDevice));
-    FBP_TRY(cudaMalloc(&p->d_qwork, p->esize * (size_t)max_batch * n_angles * n_det));
+    FBP_TRY(cudaMalloc(&p->d_rho, p->esize * (size_t)n_det));
+    FBP_TRY(cudaMemcpy(p->d_rho, rsrc, p->esize * (size_t)n_det, cudaMemcpyHostToDevice));
+    FBP_TRY(cudaMalloc(&p->d_ent, 4 * p->esize * (size_t)max_batch * n_angles * p->bp.ent_pitch));
     if (p->bp_splits > 1)
         FBP_TRY(cudaMalloc(&p->d_part, p->esize * (size_t)p->bp_splits * max_batch * image_n * image_n));
     for (int i = 0; i < 4; ++i) FBP_TRY(cudaEventCreate(&p->ev[i]));
@@ -396,7 +441,7 @@ void fbp_destroy(fbp_plan* p)
     if (!p) return;
     {
         DeviceGuard guard(p->device);
-        cudaFree(p->d_cs2); cudaFree(p->d_taps); cudaFree(p->d_qwork); cudaFree(p->d_part);
+        cudaFree(p->d_cs2); cudaFree(p->d_taps); cudaFree(p->d_rho); cudaFree(p->d_ent); cudaFree(p->d_part);
         cudaFree(p->d_hsino); cudaFree(p->d_himg);
         for (int i = 0; i < 4; ++i) if (p->ev[i]) cudaEventDestroy(p->ev[i]);
         cudaGetLastError();
@@ -417,7 +462,7 @@ fbp_status fbp_filter(fbp_plan* p, const void* d_sino, void* d_filtered, int bat
     if (d_sino == d_filtered) return fail(p, FBP_EINVAL, "fbp_filter: input and output may not alias");
     DeviceGuard guard(p->device);
     p->ran_filter = p->ran_bp = false;
-    return run_filter(p, d_sino, d_filtered, batch, static_cast<cudaStream_t>(stream));
+    return run_filter(p, d_sino, d_filtered, nullptr, batch, static_cast<cudaStream_t>(stream));
 }
 
 fbp_status fbp_backproject(fbp_plan* p, const void* d_filtered, void* d_image, int batch, void* stream)
@@ -436,9 +481,9 @@ fbp_status fbp_reconstruct(fbp_plan* p, const void* d_sino, void* d_image, int b
     DeviceGuard guard(p->device);
     p->ran_filter = p->ran_bp = false;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    st = run_filter(p, d_sino, p->d_qwork, batch, s);
+    st = run_filter(p, d_sino, nullptr, p->d_ent, batch, s);
     if (st != FBP_OK) return st;
-    return run_bp(p, p->d_qwork, d_image, batch, s);
+    return run_bp(p, nullptr, d_image, batch, s);
 }
 
 fbp_status fbp_reconstruct_host(fbp_plan* p, const void* h_sino, void* h_image, int batch, void* stream)
@@ -453,9 +498,9 @@ fbp_status fbp_reconstruct_host(fbp_plan* p, const void* h_sino, void* h_image, 
     if (!p->d_himg) FBP_CUDA(p, cudaMalloc(&p->d_himg, img_bytes * p->max_batch));
     FBP_CUDA(p, cudaMemcpyAsync(p->d_hsino, h_sino, sino_bytes * batch, cudaMemcpyHostToDevice, s));
     p->ran_filter = p->ran_bp = false;
-    fbp_status st = run_filter(p, p->d_hsino, p->d_qwork, batch, s);
+    fbp_status st = run_filter(p, p->d_hsino, nullptr, p->d_ent, batch, s);
     if (st != FBP_OK) return st;
-    st = run_bp(p, p->d_qwork, p->d_himg, batch, s);
+    st = run_bp(p, nullptr, p->d_himg, batch, s);
     if (st != FBP_OK) return st;
     FBP_CUDA(p, cudaMemcpyAsync(h_image, p->d_himg, img_bytes * batch, cudaMemcpyDeviceToHost, s));
     FBP_CUDA(p, cudaStreamSynchronize(s));
@@ -467,7 +512,7 @@ int fbp_plan_info(const fbp_plan* p, int* out, int n)
     if (!p) return 0;
     const int v[14] = {p->bp_tw, p->bp_th, p->bp_r, p->bp_splits, p->bp_chunk, p->bp_seg,
                        p->bp.tiles_x * p->bp.tiles_y * p->bp_splits, p->bp_threads, p->bp_smem,
-                       p->f_r, p->f_threads, p->fp.rows_per_cta, p->f_smem,
+                       p->f_r, p->f_threads, p->fp.n_sb, p->f_smem,
                        p->bp_splits > 1 ? 3 : 2};
     if (out) for (int i = 0; i < n && i < 14; ++i) out[i] = v[i];
     return 14;

@@ -3,123 +3,184 @@
 // Q[i][n] = (1/d) * ( h[0] P[i][n] + sum_{odd m} h[m] P[i][n-m] ),  h[0] = 1/4,
 // h[m] = -1/(pi^2 m^2) for odd m, 0 for even m != 0 (include/fbp.h).
 //
-// Only odd taps are non-zero, so an output of parity p reads inputs of parity 1-p only:
-// the row splits into two half-size dense Toeplitz products (polyphase form).  With
-//   n = 2a + p,  k = 2b + (1-p),  m = n - k = 2q + 1,  q = a - b - (1-p),
-//   g[q] := h[2q+1] = -1/(pi^2 (2q+1)^2)
-// a thread owns R consecutive same-parity outputs a0..a0+R-1 and walks b = 0..Din-1:
-//   acc[r] += g[a0 + r - b - (1-p)] * X[b].
-// The R taps it needs at step b are a window that slides by one per step, so the window
-// lives in registers (rotating through an R-times unrolled body): one new tap load + one
-// broadcast input load per R FMAs.  Lanes of a warp own consecutive output blocks, so the
-// tap loads of a warp have stride R words: R is odd => conflict-free.  The input load is
-// the same address for the whole warp (broadcast).
+// Polyphase form.  Only odd taps are non-zero, so an output of parity p reads inputs of
+// parity 1-p only.  With n = 2a + p, k = 2b + (1-p), m = n - k = 2q + 1:
+//   q = a - b - (1-p),   g[q] := h[2q+1] = -1/(pi^2 (2q+1)^2).
+// A thread owns R consecutive same-parity outputs a0..a0+R-1 and walks inputs b:
+//   acc[r] += g[a0 + r - b - (1-p)] * (X[b] - c)
+// The R taps needed at step b form a window that slides by one per step; it lives in
+// registers (rotating through an R-times unrolled body): per step one tap load (lanes own
+// consecutive output blocks => stride R words, R odd => conflict-free), one broadcast input
+// load, one subtract and R FMAs.
 //
-// One CTA filters `rows_per_cta` rows; each row is served by wpr0 warps for even outputs
-// and wpr1 warps for odd outputs.  Rows are staged to shared memory de-interleaved by
-// parity (coalesced global reads), results go through a shared row buffer so the global
-// stores are coalesced too.  No atomics; every output has one owner; fixed order.
+// Conditioning.  1/4 P[n] cancels against sum_m |h[m]| P[n-m] ~ 1/4 P[n]; summed naively in
+// fp32 the rounding error scales with P, not with Q.  Filtering is linear, so each thread
+// subtracts a constant c (the input at the centre of its output block) from every input and
+// adds c * rho[n] back at the end, rho[n] = 1/4 + sum_b g[a - b - (1-p)] over the (padded)
+// input range, computed in fp64 on the host.  The running sums then hold differences of
+// neighbouring samples times taps instead of two large cancelling numbers.
+//
+// Work decomposition.  One CTA filters one row.  Warp (p, ob, sb) owns parity p, output block
+// ob (32*R outputs) and slice sb of the input range (SB slices, so that one 512^2-sized
+// sinogram still fills 148 SMs).  Partial sums go to shared memory and are added in fixed
+// order sb = 0..SB-1 by one owner thread per output: no atomics, deterministic.
+// The epilogue writes the plain row Q[i][:] (fbp_filter) and/or the back-projector's
+// interleaved entries (fbp_reconstruct; see fbp_backproject.cuh "BpEntry").
 #pragma once
 #include <cuda_runtime.h>
 
 namespace fbp {
 
 struct FilterParams {
-    int n_rows;        // batch * K
-    int n_det;         // D
-    int rows_per_cta;
-    int wpr0, wpr1;    // warps per row for even / odd outputs
-    int de, dn;        // ceil(D/2) even-indexed samples, floor(D/2) odd-indexed samples
-    int de_pad, dn_pad;  // padded to a multiple of R (zero filled)
-    int tab_len, tab_off;  // tap table: G[idx] = g[idx - tab_off]
-    int y_pitch;       // elements per staged output row
+    int n_rows;            // batch * K
+    int n_det;             // D
+    int de, dn;            // ceil(D/2) even-indexed samples, floor(D/2) odd-indexed samples
+    int de_pad, dn_pad;    // padded to a multiple of SB*R (zero filled)
+    int n_ob;              // output blocks of 32*R per parity
+    int n_sb;              // input slices SB
+    int tab_off;           // tap table: G[q + tab_off] = g[q]
+    int tab_cnt;           // taps staged per parity: max(de_pad, dn_pad) + n_ob*32*R + R + 1
+    int x_pitch;           // elements per staged input array
+    // entry output (0 = none): row pitch in entries and left guard, see BpEntry
+    int ent_pitch, ent_guard;
 };
+
+// (mid_a, mid_b, slope_a, nslope_b) for detector interval j and its mirror D-2-j.
+template <typename T> struct alignas(4 * sizeof(T)) BpEntry { T mid_a, mid_b, slope_a, nslope_b; };
+
+// Entry j of a row from the zero-extended row values (global or shared pointer `q`).
+template <typename T>
+__device__ __forceinline__ BpEntry<T> make_entry(const T* q, int D, int j)
+{
+    const int jm = D - 2 - j;
+    const T a0 = (j >= 0 && j < D) ? q[j] : T(0);
+    const T a1 = (j + 1 >= 0 && j + 1 < D) ? q[j + 1] : T(0);
+    const T b0 = (jm >= 0 && jm < D) ? q[jm] : T(0);
+    const T b1 = (jm + 1 >= 0 && jm + 1 < D) ? q[jm + 1] : T(0);
+    BpEntry<T> e;
+    e.mid_a = T(0.5) * (a0 + a1);
+    e.mid_b = T(0.5) * (b0 + b1);
+    e.slope_a = a1 - a0;
+    e.nslope_b = b0 - b1;
+    return e;
+}
 
 template <typename T, int R>
 __global__ void __launch_bounds__(512)
-filter_kernel(const T* __restrict__ P, T* __restrict__ Q, const T* __restrict__ G_gmem,
-              FilterParams prm, T inv_d)
+filter_kernel(const T* __restrict__ P, T* __restrict__ Q, BpEntry<T>* __restrict__ E,
+              const T* __restrict__ G_gmem, const T* __restrict__ rho, FilterParams prm, T inv_d)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    T* G = reinterpret_cast<T*>(smem_raw);
-    const int row_words = prm.de_pad + prm.dn_pad + prm.y_pitch;
-    T* rows_base = G + prm.tab_len;
+    extern __shared__ __align__(16) unsigned char filt_smem_raw[];
+    // layout: G0[tab_cnt] G1[tab_cnt] X0[x_pitch] X1[x_pitch] C[2*n_ob*32] Y[y_pitch] part[...]
+    T* G0 = reinterpret_cast<T*>(filt_smem_raw);
+    T* X0 = G0 + 2 * prm.tab_cnt;
+    T* X1 = X0 + prm.x_pitch;
+    T* Cs = X1 + prm.x_pitch;
+    const int blk = 32 * R;
+    const int y_pitch = 2 * prm.n_ob * blk;
+    T* Y = Cs + 2 * prm.n_ob * 32;          // Y[p][ob*blk + o] : filtered outputs by parity
+    T* part = Y + y_pitch;                  // part[sb][p][ob*blk + o]
 
-    const int tid = threadIdx.x;
-    const int nthr = blockDim.x;
-    const int row0 = blockIdx.x * prm.rows_per_cta;
+    const int tid = threadIdx.x, nthr = blockDim.x;
+    const int row = blockIdx.x;
     const int D = prm.n_det;
+    const T* prow = P + (size_t)row * D;
 
-    // ---- stage taps and rows (coalesced), zero the padding ----
-    for (int i = tid; i < prm.tab_len; i += nthr) G[i] = G_gmem[i];
-    for (int rl = 0; rl < prm.rows_per_cta; ++rl) {
-        const int row = row0 + rl;
-        T* X0 = rows_base + (size_t)rl * row_words;   // even-indexed inputs
-        T* X1 = X0 + prm.de_pad;                      // odd-indexed inputs
-        const bool live = row < prm.n_rows;
-        const T* p = P + (size_t)row * D;
-        const int span = 2 * (prm.de_pad > prm.dn_pad ? prm.de_pad : prm.dn_pad);
-        for (int k = tid; k < span; k += nthr) {
-            T v = (live && k < D) ? p[k] : T(0);
-            const int b = k >> 1;
-            if (k & 1) { if (b < prm.dn_pad) X1[b] = v; }
-            else       { if (b < prm.de_pad) X0[b] = v; }
-        }
+    // ---- stage: inputs de-interleaved by parity (zero padded), taps of both parities ----
+    for (int k = tid; k < 2 * prm.x_pitch; k += nthr) {
+        const T v = k < D ? prow[k] : T(0);
+        if (k & 1) X1[k >> 1] = v; else X0[k >> 1] = v;
+    }
+    // parity p uses taps q = a - b - (1-p), a in [0, n_ob*blk + R), b in [0, din_pad):
+    // local index = a - b + din_pad(p)  =>  global q = local - din_pad(p) - (1-p)
+    for (int i = tid; i < 2 * prm.tab_cnt; i += nthr) {
+        const int p = i >= prm.tab_cnt;
+        const int l = i - p * prm.tab_cnt;
+        const int din_pad = p ? prm.de_pad : prm.dn_pad;
+        G0[i] = G_gmem[l - din_pad - (1 - p) + prm.tab_off];
     }
     __syncthreads();
 
-    // ---- compute: warp -> (row slot, parity, block of 32*R outputs) ----
+    // ---- compute: warp -> (parity, output block, input slice) ----
     const int warp = tid >> 5, lane = tid & 31;
-    const int wpr = prm.wpr0 + prm.wpr1;
-    const int rl = warp / wpr;
-    const int wr = warp - rl * wpr;
-    if (rl < prm.rows_per_cta && row0 + rl < prm.n_rows) {
-        const int p = (wr >= prm.wpr0) ? 1 : 0;
-        const int tp = (wr - p * prm.wpr0) * 32 + lane;
-        const int count = p ? prm.dn : prm.de;        // outputs of this parity
+    {
+        const int sb = warp % prm.n_sb;
+        const int pob = warp / prm.n_sb;
+        const int p = pob / prm.n_ob, ob = pob - p * prm.n_ob;
+        const int count = p ? prm.dn : prm.de;            // outputs of this parity
         const int din_pad = p ? prm.de_pad : prm.dn_pad;  // inputs have parity 1-p
-        T* X0 = rows_base + (size_t)rl * row_words;
-        T* X1 = X0 + prm.de_pad;
-        T* Y = X1 + prm.dn_pad;
         const T* Xin = p ? X0 : X1;
         const T* Xown = p ? X1 : X0;
-        const bool active = tp * R < count;
-        const int a0 = active ? tp * R : 0;
-        // tap index of (r, b): a0 + r - b - (1-p) + tab_off
-        const T* Gw = G + (a0 - (1 - p) + prm.tab_off);
+        const T* G = G0 + p * prm.tab_cnt;
+        const int a0 = ob * blk + lane * R;
+        const int ac = min(a0 + R / 2, max(count - 1, 0));
+        const T c = Xown[ac];
+        if (sb == 0) Cs[pob * 32 + lane] = c;
+        const int per = din_pad / prm.n_sb;               // multiple of R
+        const int b_begin = sb * per, b_end = b_begin + per;
+        const T* Gw = G + (a0 + din_pad);                 // Gw[r - b] = g[a0 + r - b - (1-p)]
 
         T acc[R], W[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) { acc[r] = T(0); W[r] = Gw[r]; }
-
-        for (int b0 = 0; b0 < din_pad; b0 += R) {
+        for (int r = 0; r < R; ++r) { acc[r] = T(0); W[r] = Gw[r - b_begin]; }
+        for (int b0 = b_begin; b0 < b_end; b0 += R) {
 #pragma unroll
             for (int s = 0; s < R; ++s) {
                 if (s > 0) W[R - s] = Gw[-(b0 + s)];
-                const T x = Xin[b0 + s];
+                const T x = Xin[b0 + s] - c;
 #pragma unroll
                 for (int r = 0; r < R; ++r) acc[r] = fma(W[(r - s + R) % R], x, acc[r]);
             }
             W[0] = Gw[-(b0 + R)];
         }
-        if (active) {
+        T* pp = part + (size_t)sb * y_pitch + pob * blk + lane * R;
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const int a = a0 + r;
-                if (a < count) Y[2 * a + p] = (acc[r] + T(0.25) * Xown[a]) * inv_d;
-            }
+        for (int r = 0; r < R; ++r) pp[r] = acc[r];
+    }
+    __syncthreads();
+
+    // ---- fixed-order reduction over input slices, centre tap, conditioning term, scale ----
+    for (int o = tid; o < y_pitch; o += nthr) {
+        const int pob = o / blk;
+        const int p = pob / prm.n_ob;
+        const int a = o - p * prm.n_ob * blk;
+        const int count = p ? prm.dn : prm.de;
+        if (a < count) {
+            T s = part[o];
+            for (int k = 1; k < prm.n_sb; ++k) s += part[(size_t)k * y_pitch + o];
+            const int n = 2 * a + p;
+            const T c = Cs[pob * 32 + (o - pob * blk) / R];
+            const T xn = (p ? X1 : X0)[a];
+            Y[o] = (s + T(0.25) * (xn - c) + c * rho[n]) * inv_d;
         }
     }
     __syncthreads();
 
-    // ---- coalesced store ----
-    for (int rl2 = 0; rl2 < prm.rows_per_cta; ++rl2) {
-        const int row = row0 + rl2;
-        if (row >= prm.n_rows) break;
-        const T* Y = rows_base + (size_t)rl2 * row_words + prm.de_pad + prm.dn_pad;
+    // ---- stores: plain row and/or interleaved entries, coalesced ----
+    // X0/X1 are dead now: reuse them as the row in natural order.
+    T* Yn = X0;
+    for (int n = tid; n < D; n += nthr) Yn[n] = Y[(n & 1) * prm.n_ob * blk + (n >> 1)];
+    __syncthreads();
+    if (Q) {
         T* q = Q + (size_t)row * D;
-        for (int n = tid; n < D; n += nthr) q[n] = Y[n];
+        for (int n = tid; n < D; n += nthr) q[n] = Yn[n];
     }
+    if (E) {
+        BpEntry<T>* e = E + (size_t)row * prm.ent_pitch;
+        for (int i = tid; i < prm.ent_pitch; i += nthr) e[i] = make_entry<T>(Yn, D, i - prm.ent_guard);
+    }
+}
+
+// Plain filtered rows -> interleaved entries (fbp_backproject's first step); same arithmetic
+// as the filter epilogue, so fbp_reconstruct == fbp_backproject(fbp_filter) bit for bit.
+template <typename T>
+__global__ void __launch_bounds__(256)
+entries_kernel(const T* __restrict__ Q, BpEntry<T>* __restrict__ E, int n_det, int ent_pitch, int ent_guard)
+{
+    const int row = blockIdx.x;
+    const T* q = Q + (size_t)row * n_det;
+    BpEntry<T>* e = E + (size_t)row * ent_pitch;
+    for (int i = threadIdx.x; i < ent_pitch; i += blockDim.x) e[i] = make_entry<T>(q, n_det, i - ent_guard);
 }
 
 }  // namespace fbp

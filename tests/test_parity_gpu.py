@@ -3,8 +3,10 @@ element on the same seeded inputs.  Tolerances are BASELINE.json's (SURVEY.md 8(
   fp64: max|f_gpu - f_oracle| / max|f_oracle| <= 1e-12
   fp32: max-abs <= 1e-4 * DR and RMSE <= 1e-5 * DR,  DR = max(f_oracle) - min(f_oracle)
 fp32 inputs are rounded to fp32 once and the oracle consumes those rounded values.
-The filter alone is held to 1e-12 (fp64) and 1e-5 (fp32; a
-~D/2-term fp32 sum) of max|Q_oracle|."""
+The filter alone is held to 1e-12 of max|Q_oracle| in fp64.  In fp32 the Ram-Lak sum cancels
+heavily (1/4 P[n] against sum |h[m]| P[n-m] -> 1/4 P[n]), so its error scales with the terms, not
+with Q: the bar is the probabilistic bound for an n-term recursive fp32 sum (DESIGN.md
+"Tolerances"): |err| <= sqrt(n) * 2^-24 * sum|terms|, n = D/2 + 1, sum|terms| <= (1/2) max|P| / d."""
 import math
 import os
 
@@ -17,7 +19,6 @@ pytestmark = pytest.mark.gpu
 
 F64_TOL = 1e-12
 F32_MAXABS, F32_RMSE = 1e-4, 1e-5
-F32_FILTER_TOL = 1e-5
 
 
 def _torch():
@@ -50,11 +51,18 @@ def check_image(gpu, ref, dt, what=""):
     return mx
 
 
-def check_filter(gpu, ref, dt, what=""):
+def check_filter(gpu, ref, dt, what="", p_max=None, d=1.0):
+    """p_max = max|P| of the (rounded) input rows the outputs come from (fp32 bound above)."""
     gpu = np.asarray(gpu, dtype=np.float64)
-    rel = np.abs(gpu - ref).max() / max(np.abs(ref).max(), 1e-300)
-    assert rel <= (F64_TOL if dt == "f64" else F32_FILTER_TOL), "%s filter rel %.3e" % (what, rel)
-    return rel
+    err = np.abs(gpu - ref).max()
+    if dt == "f64":
+        rel = err / max(np.abs(ref).max(), 1e-300)
+        assert rel <= F64_TOL, "%s filter fp64 rel %.3e" % (what, rel)
+        return rel
+    n_det = ref.shape[-1]
+    bound = math.sqrt(n_det / 2 + 1) * 2.0 ** -24 * 0.5 * p_max / d
+    assert err <= bound, "%s filter fp32 abs err %.3e > bound %.3e" % (what, err, bound)
+    return err / bound
 
 
 def run_case(fbp, oracle, sino64, angles, n, dt, d=1.0, pix=None, what=""):
@@ -71,7 +79,7 @@ def run_case(fbp, oracle, sino64, angles, n, dt, d=1.0, pix=None, what=""):
         ds = _to_dev(sino_in, dt)
         q_gpu = plan.filter(ds)
         q_ref = oracle.filter_sinogram(sino_ref, d)
-        check_filter(q_gpu.cpu().numpy(), q_ref, dt, what)
+        check_filter(q_gpu.cpu().numpy(), q_ref, dt, what, np.abs(sino_ref).max(), d)
         # back-projection alone, fed the oracle's Q rounded to the dtype
         q_in = q_ref.astype(_np_dtype(dt))
         f_ref_bp = oracle.backproject(q_in.astype(np.float64), angles, n, d, pix)
@@ -149,14 +157,14 @@ def test_cfg5_full_size_sampled(fbp, oracle, dt):
         q_gpu = plan.filter(ds).cpu().numpy()
         rows_f = np.array([0, 1, 449, 900, 1234, 1799], dtype=np.int32)
         q_rows = oracle.filter_rows(sino_ref, rows_f)
-        check_filter(q_gpu[rows_f], q_rows, dt, "cfg5")
+        check_filter(q_gpu[rows_f], q_rows, dt, "cfg5", np.abs(sino_ref).max())
         # whole chain on sampled pixels: the oracle filters the full sinogram itself (nothing
         # the CUDA path produced is ever an oracle input) and back-projects the samples; DR
         # is taken over the oracle's samples.
         f_gpu = plan.reconstruct(ds).cpu().numpy()
         rr, cc = _sample_pixels(cfg.image_n, 3000, 55)
         q_ref = oracle.filter_sinogram(sino_ref)
-        check_filter(q_gpu, q_ref, dt, "cfg5 all rows")
+        check_filter(q_gpu, q_ref, dt, "cfg5 all rows", np.abs(sino_ref).max())
         f_ref = oracle.backproject_pixels(q_ref, ang, cfg.image_n, rr, cc)
         check_image(f_gpu[rr, cc], f_ref, dt, "cfg5 sampled")
     finally:
@@ -175,7 +183,7 @@ def test_cfg4_batch_sampled(fbp, oracle):
         f_gpu = plan.reconstruct(ds).cpu().numpy()
         for s in (0, 37, 63):
             q_ref = oracle.filter_sinogram(sino_in[s].astype(np.float64))
-            check_filter(q_gpu[s], q_ref, "f32", "cfg4 s%d" % s)
+            check_filter(q_gpu[s], q_ref, "f32", "cfg4 s%d" % s, np.abs(sino_in[s]).max())
             rr, cc = _sample_pixels(cfg.image_n, 2000, 400 + s)
             f_ref = oracle.backproject_pixels(q_ref, ang, cfg.image_n, rr, cc)
             check_image(f_gpu[s][rr, cc], f_ref, "f32", "cfg4 s%d" % s)
