@@ -46,11 +46,12 @@ struct fbp_plan {
     void* d_rho = nullptr;      // [D] dtype: conditioning term of the filter (fbp_filter.cuh)
     void* d_ent = nullptr;      // [max_batch][K][ent_pitch] BpEntry: back-projector operands
     void* d_part = nullptr;     // [S][max_batch][N][N] partial images when S > 1
+    int* d_tickets = nullptr;   // [max_batch][tiles] arrival counters when S > 1 (self re-arming)
     void* d_hsino = nullptr;    // host-path staging (lazy)
     void* d_himg = nullptr;
 
     // back-projection configuration
-    int bp_variant = 0;         // 0: 32x32 tile, R=8, WY=4;  1: 32x16, R=4, WY=4;  2: 32x16, R=8, WY=2
+    int bp_variant = 0;         // index into kBpVariants: (R, WY, WA)
     int bp_tw = 32, bp_th = 32, bp_r = 8, bp_threads = 128;
     int bp_splits = 1, bp_chunk = 1, bp_seg = 0, bp_smem = 0;
     fbp::BpParams bp{};
@@ -142,23 +143,49 @@ void configure_filter(fbp_plan* p)
     f.x_pitch = round_up(din_max, 4);
     p->f_threads = 2 * f.n_ob * sb * 32;
     const size_t words = 2 * (size_t)f.tab_cnt + 2 * (size_t)f.x_pitch + 2 * (size_t)f.n_ob * 32 +
-                         (size_t)(1 + sb) * 2 * f.n_ob * 32 * R;
+                         (size_t)(1 + sb) * 2 * f.n_ob * 32 * R + (size_t)(p->bp.ent_pitch + 2);
     p->f_smem = (int)(words * p->esize + 16);
 }
 
 // ---- back-projection launch configuration ------------------------------------------
+// (R, WY, WA) instantiations of backproject_kernel, see launch_bp
+constexpr int kNumBpVariants = 11;
+constexpr int kBpVariants[kNumBpVariants][3] = {
+    {8, 4, 1}, {4, 4, 1}, {4, 1, 4}, {5, 1, 4}, {6, 1, 4}, {7, 1, 4}, {8, 1, 4},
+    {4, 1, 8}, {6, 1, 8}, {7, 1, 8}, {8, 1, 8}};
 void configure_bp(fbp_plan* p, const std::vector<double>& cs)
 {
-    p->bp_variant = env_int("FBP_BP_VARIANT", 0);
-    if (p->bp_variant < 0 || p->bp_variant > 2) p->bp_variant = 0;
-    switch (p->bp_variant) {
-        case 0: p->bp_th = 32; p->bp_r = 8; p->bp_threads = 128; break;
-        case 1: p->bp_th = 16; p->bp_r = 4; p->bp_threads = 128; break;
-        default: p->bp_th = 16; p->bp_r = 8; p->bp_threads = 64; break;
-    }
     const int N = p->N, K = p->K;
-    const int tiles_x = (N + p->bp_tw - 1) / p->bp_tw;
     const int half_rows = (N + 1) / 2;  // primary (top) half; the mirror pixels come for free
+    const int tiles_x = (N + p->bp_tw - 1) / p->bp_tw;
+    // variant = (R rows per thread, WY warps along y, WA angle groups): tile 32 x (R*WY) primary pixels
+    int v = env_int("FBP_BP_VARIANT", -1);
+    if (v < 0 || v >= kNumBpVariants) {
+        // Small launches (one 512^2 slice is 16 column strips x 256 primary rows) are chosen to fill
+        // 148 SMs evenly: short tiles of R rows with 4 angle groups, R picked so that the number of
+        // CTAs is as close as possible to a whole number of waves.  Large launches take the 32x32
+        // tile (a third of the L2->shared staging traffic per update).
+        const long big = (long)tiles_x * ((half_rows + 31) / 32) * p->max_batch;
+        if (big >= 8L * kNumSm) {
+            v = 0;
+        } else {
+            double best = -1.0;
+            v = 3;
+            for (int cand = 2; cand <= 6; ++cand) {
+                const int th = kBpVariants[cand][0] * kBpVariants[cand][1];
+                const long ctas = (long)tiles_x * ((half_rows + th - 1) / th) * p->max_batch;
+                const long waves = (ctas + 4L * kNumSm - 1) / (4L * kNumSm);   // 4 CTAs of 4 warps per SM
+                const double fill = (double)ctas / (double)(waves * 4L * kNumSm);
+                const double waste = (double)half_rows / (double)(((half_rows + th - 1) / th) * th);
+                const double score = fill * waste * (1.0 - 0.15 / th);         // taller tiles stage less
+                if (score > best) { best = score; v = cand; }
+            }
+        }
+    }
+    p->bp_variant = v;
+    p->bp_r = kBpVariants[v][0];
+    p->bp_th = kBpVariants[v][0] * kBpVariants[v][1];
+    p->bp_threads = 32 * (kBpVariants[v][1] * kBpVariants[v][2] + 1);   // + the producer warp
     const int tiles_y = (half_rows + p->bp_th - 1) / p->bp_th;
     double ext = 0.0;
     for (int i = 0; i < K; ++i) {
@@ -184,19 +211,23 @@ void configure_bp(fbp_plan* p, const std::vector<double>& cs)
         }
     }
     if (S > K) S = K;
+    if (S > 64) S = 64;
     if (S < 1) S = 1;
     p->bp_splits = S;
     const int per = (K + S - 1) / S;
 
     const size_t entry = 4 * p->esize, rec = 4 * p->esize;
     const size_t per_angle = (size_t)p->bp_seg * entry + rec;
-    int budget = env_int("FBP_BP_SMEM", 24 * 1024);
+    int budget = env_int("FBP_BP_SMEM", 36 * 1024);
     int chunk = env_int("FBP_BP_CHUNK", 0);
-    if (chunk <= 0) chunk = (int)(budget / per_angle);
+    if (chunk <= 0) chunk = (int)(budget / (fbp::kBpStages * per_angle));
     if (chunk > per) chunk = per;
     if (chunk < 1) chunk = 1;
     p->bp_chunk = chunk;
-    p->bp_smem = (int)(per_angle * chunk + 16 + 128);
+    size_t seg_bytes = fbp::kBpStages * (size_t)p->bp_seg * entry * chunk;
+    const size_t red_bytes = (size_t)(kBpVariants[v][2] - 1) * 2 * p->bp_r * (32 * kBpVariants[v][1]) * p->esize;
+    if (seg_bytes < red_bytes) seg_bytes = red_bytes;          // in-CTA reduction reuses the stages
+    p->bp_smem = (int)(64 + fbp::kBpStages * rec * chunk + 128 + seg_bytes);
 
     fbp::BpParams& b = p->bp;
     b.n_angles = K; b.n_det = p->D; b.image_n = N;
@@ -224,7 +255,7 @@ cudaError_t launch_filter_r(const fbp_plan* p, const void* sino, void* filt, voi
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, p->f_smem);
     if (e != cudaSuccess) return e;
     kern<<<f.n_rows, p->f_threads, p->f_smem, st>>>(static_cast<const T*>(sino), static_cast<T*>(filt),
-                                                     static_cast<fbp::BpEntry<T>*>(ent),
+                                                     static_cast<uint4*>(ent),
                                                      static_cast<const T*>(p->d_taps),
                                                      static_cast<const T*>(p->d_rho), f, (T)(1.0 / p->d));
     return cudaGetLastError();
@@ -247,21 +278,25 @@ cudaError_t launch_filter(const fbp_plan* p, const void* sino, void* filt, void*
 template <typename T>
 cudaError_t launch_entries(const fbp_plan* p, const void* filt, int batch, cudaStream_t st)
 {
-    fbp::entries_kernel<T><<<batch * p->K, 256, 0, st>>>(static_cast<const T*>(filt),
-                                                         static_cast<fbp::BpEntry<T>*>(p->d_ent), p->D,
-                                                         p->bp.ent_pitch, p->bp.ent_guard);
+    const size_t smem = (size_t)(p->bp.ent_pitch + 2) * sizeof(T);
+    auto kern = fbp::entries_kernel<T>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    kern<<<batch * p->K, 256, smem, st>>>(static_cast<const T*>(filt), static_cast<uint4*>(p->d_ent), p->D,
+                                          p->bp.ent_pitch, p->bp.ent_guard);
     return cudaGetLastError();
 }
 
-template <typename T, int R, int WY>
-cudaError_t launch_bp_v(const fbp_plan* p, void* out, int batch, cudaStream_t st)
+template <typename T, int R, int WY, int WA>
+cudaError_t launch_bp_v(const fbp_plan* p, void* image, int batch, cudaStream_t st)
 {
-    auto kern = fbp::backproject_kernel<T, R, WY>;
+    auto kern = fbp::backproject_kernel<T, R, WY, WA>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, p->bp_smem);
     if (e != cudaSuccess) return e;
     dim3 grid(p->bp.tiles_x * p->bp.tiles_y, p->bp_splits, batch);
-    kern<<<grid, 32 * WY, p->bp_smem, st>>>(static_cast<const fbp::BpEntry<T>*>(p->d_ent), static_cast<T*>(out),
-                                            p->d_cs2, p->bp, batch);
+    kern<<<grid, 32 * (WY * WA + 1), p->bp_smem, st>>>(static_cast<const uint4*>(p->d_ent), static_cast<T*>(image),
+                                            static_cast<const double2*>(p->d_cs2), static_cast<T*>(p->d_part),
+                                            p->d_tickets, p->bp);
     return cudaGetLastError();
 }
 
@@ -269,20 +304,19 @@ cudaError_t launch_bp_v(const fbp_plan* p, void* out, int batch, cudaStream_t st
 template <typename T>
 cudaError_t launch_bp(const fbp_plan* p, void* image, int batch, cudaStream_t st)
 {
-    void* out = p->bp_splits > 1 ? p->d_part : image;
-    cudaError_t e;
     switch (p->bp_variant) {
-        case 0: e = launch_bp_v<T, 8, 4>(p, out, batch, st); break;
-        case 1: e = launch_bp_v<T, 4, 4>(p, out, batch, st); break;
-        default: e = launch_bp_v<T, 8, 2>(p, out, batch, st); break;
+        case 0: return launch_bp_v<T, 8, 4, 1>(p, image, batch, st);
+        case 1: return launch_bp_v<T, 4, 4, 1>(p, image, batch, st);
+        case 2: return launch_bp_v<T, 4, 1, 4>(p, image, batch, st);
+        case 3: return launch_bp_v<T, 5, 1, 4>(p, image, batch, st);
+        case 4: return launch_bp_v<T, 6, 1, 4>(p, image, batch, st);
+        case 5: return launch_bp_v<T, 7, 1, 4>(p, image, batch, st);
+        case 6: return launch_bp_v<T, 8, 1, 4>(p, image, batch, st);
+        case 7: return launch_bp_v<T, 4, 1, 8>(p, image, batch, st);
+        case 8: return launch_bp_v<T, 6, 1, 8>(p, image, batch, st);
+        case 9: return launch_bp_v<T, 7, 1, 8>(p, image, batch, st);
+        default: return launch_bp_v<T, 8, 1, 8>(p, image, batch, st);
     }
-    if (e != cudaSuccess || p->bp_splits == 1) return e;
-    const size_t n = (size_t)batch * p->N * p->N;
-    int blocks = (int)((n + 255) / 256);
-    if (blocks > kNumSm * 8) blocks = kNumSm * 8;
-    fbp::reduce_kernel<T><<<blocks, 256, 0, st>>>(static_cast<const T*>(p->d_part), static_cast<T*>(image), n,
-                                                 p->bp_splits, (T)p->bp.scale);
-    return cudaGetLastError();
 }
 
 bool aligned16(const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15u) == 0; }
@@ -374,8 +408,8 @@ fbp_status fbp_create(fbp_plan** out, int n_angles, int n_det, const double* ang
         cs[2 * i] = std::cos(angles_rad[i]) * ratio;
         cs[2 * i + 1] = std::sin(angles_rad[i]) * ratio;
     }
-    configure_filter(p);
     configure_bp(p, cs);
+    configure_filter(p);   // after configure_bp: needs the entry pitch
 
     auto bail = [&](fbp_status st) { std::string m = p->err; fbp_destroy(p); g_create_error = m; return st; };
     if (p->f_threads > 512) { p->err = "n_det too large for the row filter (more than 512 threads per row)"; return bail(FBP_EUNSUPPORTED); }
@@ -428,8 +462,12 @@ fbp_status fbp_create(fbp_plan** out, int n_angles, int n_det, const double* ang
     FBP_TRY(cudaMalloc(&p->d_rho, p->esize * (size_t)n_det));
     FBP_TRY(cudaMemcpy(p->d_rho, rsrc, p->esize * (size_t)n_det, cudaMemcpyHostToDevice));
     FBP_TRY(cudaMalloc(&p->d_ent, 4 * p->esize * (size_t)max_batch * n_angles * p->bp.ent_pitch));
-    if (p->bp_splits > 1)
+    if (p->bp_splits > 1) {
+        const size_t nt = (size_t)max_batch * p->bp.tiles_x * p->bp.tiles_y;
         FBP_TRY(cudaMalloc(&p->d_part, p->esize * (size_t)p->bp_splits * max_batch * image_n * image_n));
+        FBP_TRY(cudaMalloc(&p->d_tickets, sizeof(int) * nt));
+        FBP_TRY(cudaMemset(p->d_tickets, 0, sizeof(int) * nt));
+    }
     for (int i = 0; i < 4; ++i) FBP_TRY(cudaEventCreate(&p->ev[i]));
 #undef FBP_TRY
     *out = p;
@@ -441,7 +479,7 @@ void fbp_destroy(fbp_plan* p)
     if (!p) return;
     {
         DeviceGuard guard(p->device);
-        cudaFree(p->d_cs2); cudaFree(p->d_taps); cudaFree(p->d_rho); cudaFree(p->d_ent); cudaFree(p->d_part);
+        cudaFree(p->d_cs2); cudaFree(p->d_taps); cudaFree(p->d_rho); cudaFree(p->d_ent); cudaFree(p->d_part); cudaFree(p->d_tickets);
         cudaFree(p->d_hsino); cudaFree(p->d_himg);
         for (int i = 0; i < 4; ++i) if (p->ev[i]) cudaEventDestroy(p->ev[i]);
         cudaGetLastError();
@@ -513,7 +551,7 @@ int fbp_plan_info(const fbp_plan* p, int* out, int n)
     const int v[14] = {p->bp_tw, p->bp_th, p->bp_r, p->bp_splits, p->bp_chunk, p->bp_seg,
                        p->bp.tiles_x * p->bp.tiles_y * p->bp_splits, p->bp_threads, p->bp_smem,
                        p->f_r, p->f_threads, p->fp.n_sb, p->f_smem,
-                       p->bp_splits > 1 ? 3 : 2};
+                       2};
     if (out) for (int i = 0; i < n && i < 14; ++i) out[i] = v[i];
     return 14;
 }

@@ -9,21 +9,33 @@
 // interpolation operands with ONE 16-byte (fp32) shared-memory load of the entry
 //   E[i][j] = ( mid[j], mid[D-2-j], slope[j], -slope[D-2-j] ),
 //   mid[j] = (Q~[j]+Q~[j+1])/2,  slope[j] = Q~[j+1]-Q~[j],  Q~ = 0 outside [0, D-1]
-// so that  value = mid_a + w slope_a  and  mirror value = mid_b + w nslope_b.
+// so that  value = mid_a + w slope_a  and  mirror value = mid_b + w nslope_b; in fp32 that is
+// one packed FFMA2 + one packed FADD2 on the (pixel, mirror) accumulator pair.
+// In fp64 the entry is split into two 16-byte planes (mids, slopes) so that consecutive
+// entries stay 16 bytes apart (a 32-byte entry would 2-way bank-conflict every LDS.128).
 // The entries are produced by the filter epilogue (fbp_reconstruct) or entries_kernel
-// (fbp_backproject) into a plan-owned buffer [batch][K][pitch] with >= L+1 zero guard
-// entries on both sides.
+// (fbp_backproject) into a plan-owned buffer [batch][K][planes][pitch] with >= L+1 zero
+// guard entries on both sides (fbp_filter.cuh, "entries").
 //
 // A CTA owns a tile of 32 x (WY*R) primary pixels and a contiguous range of angles (split s
-// of S).  Angles are processed in chunks; for each angle of a chunk lane a of warp 0
-// computes, in fp64, the tile-local base b = u(tile origin) - j0 - 1/2 (fp32 coordinates
-// stay below 64: ulp <= 3.8e-6) and issues one TMA bulk copy (cp.async.bulk, completion on an
-// mbarrier) of the L entries starting at j0 into shared memory.
+// of S).  Its warps form WA groups of WY warps; group g takes every WA-th angle, so one small
+// tile still keeps 4-8 warps busy, and the WA partial sums are added in fixed order g = 0..WA-1
+// through shared memory at the end.  Angles are staged in chunks through a two-stage ring:
+// while the CTA works on chunk k, lane a of warp 0 computes for each angle of chunk k+1, in
+// fp64, the tile-local base b = u(tile origin) - j0 - 1/2 (fp32 coordinates stay below 64:
+// ulp <= 3.8e-6) and issues one TMA bulk copy (cp.async.bulk, completion on an mbarrier) of
+// the L entries starting at j0 into the other stage.
 // Per update pair:  u' = b + lx cos + ly sin;  t = u' + M (M = 1.5*2^23 | 1.5*2^52, round to
 // nearest);  e = bits(t) - bits(M);  w = u' - (t - M);  one LDS.128;  2 FMA + 2 ADD.
 // A tie in the rounding picks either neighbouring interval with the same interpolated value.
-// One owner per pixel, ascending angles, no atomics => bit-identical runs.  With S > 1 the S
-// partial images go to scratch and reduce_kernel adds them in fixed order s = 0..S-1.
+// One owner per pixel, ascending angles => bit-identical runs.  With S > 1 (one small slice
+// would otherwise leave most of the 148 SMs idle) the S CTAs of a tile each write their
+// partial tile to a scratch image [S][batch][N][N] and take a ticket (one atomicAdd per CTA on
+// a per-tile counter -- ordering only, never data); the CTA that draws the last ticket adds the
+// S partials in fixed order s = 0..S-1, scales by pi/K and stores the final pixels.  The sum
+// order does not depend on which CTA arrives last, so the output bytes do not either.
+// (A thread-block cluster + DSMEM reduction was measured first: clusters of 8 leave whole SMs
+// without work on B200 -- sm__cycles_active.min = 0 -- and ran 20 % slower.)
 #pragma once
 #include <cuda_runtime.h>
 #include <cstdint>
@@ -73,6 +85,10 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned byt
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(unsigned bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
 {
     asm volatile(
@@ -91,66 +107,116 @@ __device__ __forceinline__ void tma_load_1d(unsigned dst, const void* src, unsig
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 
-template <typename T> struct EntryLoad;
-template <> struct EntryLoad<float> {
-    __device__ static void ld(unsigned addr, float& ma, float& mb, float& sa, float& sb)
+
+// ---- the per-update arithmetic: (pixel, mirror pixel) accumulator pair ---------------------
+// fp32: packed pair in one 64-bit register; LDS.128 -> (mids, slopes) as two packed pairs;
+//       t = slopes * (w, w) + mids  (FFMA2, scalar w broadcast);  acc += t  (FADD2).
+// fp64: two 16-byte planes -> two LDS.128; scalar DFMA + DADD per pixel.
+template <typename T> struct PairAcc;
+template <> struct PairAcc<float> {
+    unsigned long long v;
+    static constexpr int kPlanes = 1;
+    __device__ __forceinline__ void zero() { v = 0ull; }
+    __device__ __forceinline__ void update(unsigned addr, unsigned /*plane_stride*/, float w)
     {
+#ifndef FBP_SCALAR_PAIR
+        unsigned long long m2, s2, w2, t;
+        asm volatile("ld.shared.v2.b64 {%0,%1}, [%2];" : "=l"(m2), "=l"(s2) : "r"(addr));
+        asm("mov.b64 %0, {%1, %1};" : "=l"(w2) : "f"(w));
+        asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(t) : "l"(s2), "l"(w2), "l"(m2));
+        asm("add.rn.f32x2 %0, %0, %1;" : "+l"(v) : "l"(t));
+#else
+        float ma, mb, sa, sb;
         asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(ma), "=f"(mb), "=f"(sa), "=f"(sb) : "r"(addr));
+        const float na = a() + fmaf(w, sa, ma), nb = b() + fmaf(w, sb, mb);
+        v = (unsigned long long)__float_as_uint(na) | ((unsigned long long)__float_as_uint(nb) << 32);
+#endif
     }
+    __device__ __forceinline__ float a() const { return __uint_as_float((unsigned)(v & 0xffffffffull)); }
+    __device__ __forceinline__ float b() const { return __uint_as_float((unsigned)(v >> 32)); }
 };
-template <> struct EntryLoad<double> {
-    __device__ static void ld(unsigned addr, double& ma, double& mb, double& sa, double& sb)
+template <> struct PairAcc<double> {
+    double va, vb;
+    static constexpr int kPlanes = 2;
+    __device__ __forceinline__ void zero() { va = 0.0; vb = 0.0; }
+    __device__ __forceinline__ void update(unsigned addr, unsigned plane_stride, double w)
     {
+        double ma, mb, sa, sb;
         asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(ma), "=d"(mb) : "r"(addr));
-        asm volatile("ld.shared.v2.f64 {%0,%1}, [%2+16];" : "=d"(sa), "=d"(sb) : "r"(addr));
+        asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(sa), "=d"(sb) : "r"(addr + plane_stride));
+        va += fma(w, sa, ma);
+        vb += fma(w, sb, mb);
     }
+    __device__ __forceinline__ double a() const { return va; }
+    __device__ __forceinline__ double b() const { return vb; }
 };
 
-// cs2: [K] pairs (cos*pix/d, sin*pix/d) in fp64.  E: entries [batch][K][ent_pitch].
-// out: image (S == 1, scaled) or partial buffer [S][batch][N][N] (S > 1, unscaled).
-template <typename T, int R, int WY>
-__global__ void __launch_bounds__(32 * WY)
-backproject_kernel(const BpEntry<T>* __restrict__ E, T* __restrict__ out, const double2* __restrict__ cs2,
-                   BpParams prm, int batch)
+// cs2: [K] pairs (cos*pix/d, sin*pix/d) in fp64.  E: 16-byte entry units [batch][K][planes][pitch].
+// Grid (tiles, S, batch).  image: [batch][N][N], fully written, scaled by pi/K.
+// part: scratch [S][batch][N][N] and tickets: [batch][tiles] zero-initialised counters (S > 1 only).
+#ifndef FBP_BP_REGCAP
+#define FBP_BP_REGCAP (sizeof(T) == 4 ? 64 : 96)
+#endif
+constexpr int kBpStages = 3;
+
+template <typename T, int R, int WY, int WA>
+__global__ void __launch_bounds__(32 * (WY * WA + 1), 65536 / (FBP_BP_REGCAP * 32 * (WY * WA + 1)))
+backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const double2* __restrict__ cs2,
+                   T* __restrict__ part, int* __restrict__ tickets, BpParams prm)
 {
     constexpr int TH = WY * R;
-    constexpr int ESZ = (int)sizeof(BpEntry<T>);
+    constexpr int NP = PairAcc<T>::kPlanes;
+    constexpr int NW = WY * WA;          // consumer warps; warp NW is the producer
+    constexpr int NS = kBpStages;
     extern __shared__ __align__(128) unsigned char bp_smem_raw[];
-    // layout: mbarrier (16 B) | rec[chunk] | seg[chunk][L]
-    const unsigned bar = smem_u32(bp_smem_raw);
-    AngleRec<T>* rec = reinterpret_cast<AngleRec<T>*>(bp_smem_raw + 16);
-    unsigned char* seg_ptr = bp_smem_raw + 16 + (size_t)prm.chunk * sizeof(AngleRec<T>);
+    // layout: full[NS], empty[NS] mbarriers (64 B) | rec[NS][chunk] | pad to 128 |
+    //         seg[NS stages][planes][chunk][L] x 16 B
+    const unsigned bar_full = smem_u32(bp_smem_raw);
+    const unsigned bar_empty = bar_full + 8u * NS;
+    AngleRec<T>* rec = reinterpret_cast<AngleRec<T>*>(bp_smem_raw + 64);
+    unsigned char* seg_ptr = bp_smem_raw + 64 + NS * (size_t)prm.chunk * sizeof(AngleRec<T>);
     seg_ptr += (128 - (reinterpret_cast<uintptr_t>(seg_ptr) & 127)) & 127;
     const unsigned seg = smem_u32(seg_ptr);
 
-    const int tid = threadIdx.x, lane = tid & 31, wy = tid >> 5;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const bool producer = warp == NW;
+    const int wy = warp % WY, wa = producer ? WA : warp / WY;
     const int tile = blockIdx.x;
     const int ty = tile / prm.tiles_x, tx = tile - ty * prm.tiles_x;
     const int split = blockIdx.y, b = blockIdx.z;
-    const int K = prm.n_angles, N = prm.image_n, L = prm.seg_len;
+    const int K = prm.n_angles, N = prm.image_n, L = prm.seg_len, S = prm.n_splits;
+    const unsigned plane_stride = (unsigned)(prm.chunk * L * 16);
+    const unsigned stage_stride = plane_stride * NP;
 
-    const int per = (K + prm.n_splits - 1) / prm.n_splits;
+    const int per = (K + S - 1) / S;
     const int a_begin = split * per;
     const int a_end = min(K, a_begin + per);
+    const int n_chunks = a_end > a_begin ? (a_end - a_begin + prm.chunk - 1) / prm.chunk : 0;
 
-    if (tid == 0) { mbar_init(bar, 1); fence_mbar_init(); }
+    if (tid == 0) {
+        for (int st = 0; st < NS; ++st) {
+            mbar_init(bar_full + 8u * st, 1);     // the producer's expect_tx arrival
+            mbar_init(bar_empty + 8u * st, NW);   // one arrival per consumer warp
+        }
+        fence_mbar_init();
+    }
     __syncthreads();
 
-    const double x0 = (double)(tx * 32) - prm.c_n;
-    const double y0 = (double)(ty * TH) - prm.c_n;
-    const BpEntry<T>* Eb = E + (size_t)b * K * prm.ent_pitch;
-
-    T acc_a[R], acc_b[R];
+    PairAcc<T> acc[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) { acc_a[r] = T(0); acc_b[r] = T(0); }
-    const T lx = (T)lane, ly = (T)(wy * R);
-    unsigned phase = 0;
+    for (int r = 0; r < R; ++r) acc[r].zero();
 
-    for (int a0 = a_begin; a0 < a_end; a0 += prm.chunk) {
-        const int na = min(prm.chunk, a_end - a0);
-        __syncthreads();  // every warp is done reading the previous chunk
-        if (wy == 0) {
-            if (lane == 0) mbar_arrive_expect_tx(bar, (unsigned)(na * L * ESZ));
+    if (producer) {
+        // ---- producer warp: per angle, the tile-local record (fp64) and one TMA bulk copy ----
+        const double x0 = (double)(tx * 32) - prm.c_n;
+        const double y0 = (double)(ty * TH) - prm.c_n;
+        const uint4* Eb = E + (size_t)b * K * NP * prm.ent_pitch;
+        for (int k = 0; k < n_chunks; ++k) {
+            const int st = k % NS;
+            if (k >= NS) mbar_wait(bar_empty + 8u * st, (unsigned)((k / NS - 1) & 1));  // stage released
+            const int a0 = a_begin + k * prm.chunk;
+            const int na = min(prm.chunk, a_end - a0);
+            const unsigned bar = bar_full + 8u * st;
             for (int a = lane; a < na; a += 32) {
                 const double2 cs = cs2[a0 + a];
                 const double ub = x0 * cs.x + y0 * cs.y + prm.c_d;
@@ -169,62 +235,136 @@ backproject_kernel(const BpEntry<T>* __restrict__ E, T* __restrict__ out, const 
                     rc.c = T(0); rc.s = T(0); rc.b = T(1);
                 }
                 rc.pad = T(0);
-                rec[a] = rc;
-                const BpEntry<T>* src = Eb + (size_t)(a0 + a) * prm.ent_pitch + (j0 + prm.ent_guard);
-                tma_load_1d(seg + (unsigned)(a * L * ESZ), src, (unsigned)(L * ESZ), bar);
+                rec[st * prm.chunk + a] = rc;
+                const uint4* src = Eb + (size_t)(a0 + a) * NP * prm.ent_pitch + (j0 + prm.ent_guard);
+#pragma unroll
+                for (int pl = 0; pl < NP; ++pl)
+                    tma_load_1d(seg + st * stage_stride + pl * plane_stride + (unsigned)(a * L * 16),
+                                src + (size_t)pl * prm.ent_pitch, (unsigned)(L * 16), bar);
             }
+            // every lane's records are written before lane 0's (releasing) arrival, so a warp
+            // that sees the phase complete also sees the records
+            __syncwarp();
+            if (lane == 0) mbar_arrive_expect_tx(bar, (unsigned)(na * L * 16 * NP));
         }
-        __syncthreads();        // rec[] visible to all warps
-        mbar_wait(bar, phase);  // all bulk copies of this chunk have landed
-        phase ^= 1u;
-
+    } else {
+        // ---- consumer warps: no block-wide barrier, only data (full) waits ----
+        const T lx = (T)lane, ly = (T)(wy * R);
         const T M = Magic<T>::m();
+        for (int k = 0; k < n_chunks; ++k) {
+            const int st = k % NS;
+            const int na = min(prm.chunk, a_end - (a_begin + k * prm.chunk));
+            mbar_wait(bar_full + 8u * st, (unsigned)((k / NS) & 1));  // chunk k has landed
+            const AngleRec<T>* rk = rec + st * prm.chunk;
+            const unsigned segk = seg + st * stage_stride - Magic<T>::kBits * 16u;  // bits(M) folded in
 #pragma unroll 2
-        for (int a = 0; a < na; ++a) {
-            const AngleRec<T> rc = rec[a];
-            // address of entry e: seg + a*L*ESZ + (bits(t) - bits(M)) * ESZ, bits(M) folded in
-            const unsigned rowbase = seg + (unsigned)(a * L * ESZ) - Magic<T>::kBits * (unsigned)ESZ;
-            const T u0 = fma(lx, rc.c, fma(ly, rc.s, rc.b));
+            for (int a = wa; a < na; a += WA) {
+                const AngleRec<T> rc = rk[a];
+                const unsigned rowbase = segk + (unsigned)(a * L * 16);
+                const T u0 = fma(lx, rc.c, fma(ly, rc.s, rc.b));
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const T u = fma((T)r, rc.s, u0);
+                    const T t = u + M;
+                    const T w = u - (t - M);
+                    acc[r].update(rowbase + Magic<T>::bits(t) * 16u, plane_stride, w);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_empty + 8u * st);   // this warp is done with stage st
+        }
+    }
+
+    // ---- in-CTA reduction over the WA angle groups, fixed order g = 0..WA-1 ----
+    T va[R], vb[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) { va[r] = acc[r].a(); vb[r] = acc[r].b(); }
+    if (WA > 1) {
+        __syncthreads();  // the last chunk has been consumed: the seg region can be reused
+        T* red = reinterpret_cast<T*>(seg_ptr);   // [WA-1][2R][32*WY]
+        const int lt = wy * 32 + lane;
+        if (wa > 0 && !producer) {
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-                const T u = fma((T)r, rc.s, u0);
-                const T t = u + M;
-                const T w = u - (t - M);
-                T ma, mb, sa, sb;
-                EntryLoad<T>::ld(rowbase + Magic<T>::bits(t) * (unsigned)ESZ, ma, mb, sa, sb);
-                acc_a[r] += fma(w, sa, ma);
-                acc_b[r] += fma(w, sb, mb);
+                red[((wa - 1) * 2 * R + r) * (32 * WY) + lt] = va[r];
+                red[((wa - 1) * 2 * R + R + r) * (32 * WY) + lt] = vb[r];
+            }
+        }
+        __syncthreads();
+        if (wa == 0) {
+            for (int g = 1; g < WA; ++g) {
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    va[r] += red[((g - 1) * 2 * R + r) * (32 * WY) + lt];
+                    vb[r] += red[((g - 1) * 2 * R + R + r) * (32 * WY) + lt];
+                }
             }
         }
     }
+    const bool owner = (wa == 0);   // group 0 (never the producer warp) holds the tile's sums and does every store below
 
     const int c = tx * 32 + lane;
-    if (c < N) {
-        const size_t img = (size_t)N * N;
-        T* o = out + ((size_t)split * batch + b) * img;
-        const T sc = (prm.n_splits == 1) ? (T)prm.scale : T(1);
+    T* img = image + (size_t)b * N * N;
+    const T sc = (T)prm.scale;
+    // pixel offsets of this thread: primary rows (base_a + r*N) and their mirrors (base_b - r*N)
+    const int row0 = ty * TH + wy * R;
+    const long long base_a = (long long)row0 * N + c;
+    const long long base_b = (long long)(N - 1 - row0) * N + (N - 1 - c);
+    auto ok_a = [&](int r) { return owner && c < N && row0 + r < prm.half_rows; };
+    auto ok_b = [&](int r) { return ok_a(r) && (N - 1 - row0 - r) >= prm.half_rows; };
+
+    if (S == 1) {
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const int row = ty * TH + wy * R + r;
-            if (row < prm.half_rows) {
-                o[(size_t)row * N + c] = acc_a[r] * sc;
-                const int mrow = N - 1 - row;
-                if (mrow >= prm.half_rows) o[(size_t)mrow * N + (N - 1 - c)] = acc_b[r] * sc;
-            }
+            if (ok_a(r)) img[base_a + (long long)r * N] = va[r] * sc;
+            if (ok_b(r)) img[base_b - (long long)r * N] = vb[r] * sc;
         }
+        return;
     }
-}
 
-// image[p] = scale * (part[0][p] + part[1][p] + ... + part[S-1][p]), fixed order.
-template <typename T>
-__global__ void reduce_kernel(const T* __restrict__ part, T* __restrict__ image, size_t n,
-                              int n_splits, T scale)
-{
-    const size_t stride = (size_t)gridDim.x * blockDim.x;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        T s = part[i];
-        for (int k = 1; k < n_splits; ++k) s += part[(size_t)k * n + i];
-        image[i] = s * scale;
+    // ---- S > 1: partial tile -> scratch, ticket, last arriver reduces in fixed order ----
+    const size_t img_elems = (size_t)N * N;
+    const size_t split_stride = (size_t)gridDim.z * img_elems;      // [S][batch][N][N]
+    T* mine = part + (size_t)split * split_stride + (size_t)b * img_elems;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        if (ok_a(r)) mine[base_a + (long long)r * N] = va[r];
+        if (ok_b(r)) mine[base_b - (long long)r * N] = vb[r];
+    }
+    __threadfence();
+    __syncthreads();
+    __shared__ int s_last;
+    if (tid == 0) {
+        int* tk = tickets + (size_t)b * gridDim.x + tile;
+        const int t = atomicAdd(tk, 1);
+        s_last = (t == S - 1);
+        if (t == S - 1) *tk = 0;   // every CTA of the tile has arrived: re-arm for the next launch
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    const T* p0 = part + (size_t)b * img_elems;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        va[r] = ok_a(r) ? __ldcg(p0 + base_a + (long long)r * N) : T(0);
+        vb[r] = ok_b(r) ? __ldcg(p0 + base_b - (long long)r * N) : T(0);
+    }
+#pragma unroll 1
+    for (int s = 1; s < S; ++s) {
+        const T* ps = p0 + (size_t)s * split_stride;
+        T ta[R], tb[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            ta[r] = ok_a(r) ? __ldcg(ps + base_a + (long long)r * N) : T(0);
+            tb[r] = ok_b(r) ? __ldcg(ps + base_b - (long long)r * N) : T(0);
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) { va[r] += ta[r]; vb[r] += tb[r]; }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        if (ok_a(r)) img[base_a + (long long)r * N] = va[r] * sc;
+        if (ok_b(r)) img[base_b - (long long)r * N] = vb[r] * sc;
     }
 }
 

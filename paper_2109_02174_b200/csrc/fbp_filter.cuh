@@ -45,29 +45,40 @@ struct FilterParams {
     int ent_pitch, ent_guard;
 };
 
-// (mid_a, mid_b, slope_a, nslope_b) for detector interval j and its mirror D-2-j.
-template <typename T> struct alignas(4 * sizeof(T)) BpEntry { T mid_a, mid_b, slope_a, nslope_b; };
+// ---- entries: the back-projector's operands (fbp_backproject.cuh) -------------------------
+// For detector interval j (between bins j and j+1 of the zero-extended row Q~) and its mirror
+// interval D-2-j:   mid_a = (Q~[j]+Q~[j+1])/2, mid_b = (Q~[D-2-j]+Q~[D-1-j])/2,
+//                   slope_a = Q~[j+1]-Q~[j],   nslope_b = Q~[D-2-j]-Q~[D-1-j].
+// Row layout in 16-byte units, index i = j + guard, i in [0, pitch), pitch = D + 2*guard:
+//   fp32: one plane   [pitch] of (mid_a, mid_b, slope_a, nslope_b)
+//   fp64: two planes  [pitch] of (mid_a, mid_b)  then  [pitch] of (slope_a, nslope_b)
+// `yz` is the row with one extra leading zero and the guards: yz[k] = Q~[k - 1 - guard],
+// k in [0, pitch + 2).  Then the mirror interval of i starts at yz[pitch - 1 - i].
+template <typename T> struct EntryPlanes { static constexpr int value = (int)sizeof(T) / 4; };
 
-// Entry j of a row from the zero-extended row values (global or shared pointer `q`).
-template <typename T>
-__device__ __forceinline__ BpEntry<T> make_entry(const T* q, int D, int j)
+__device__ __forceinline__ void store_entry(uint4* erow, int /*pitch*/, int i, float ma, float mb, float sa, float sb)
 {
-    const int jm = D - 2 - j;
-    const T a0 = (j >= 0 && j < D) ? q[j] : T(0);
-    const T a1 = (j + 1 >= 0 && j + 1 < D) ? q[j + 1] : T(0);
-    const T b0 = (jm >= 0 && jm < D) ? q[jm] : T(0);
-    const T b1 = (jm + 1 >= 0 && jm + 1 < D) ? q[jm + 1] : T(0);
-    BpEntry<T> e;
-    e.mid_a = T(0.5) * (a0 + a1);
-    e.mid_b = T(0.5) * (b0 + b1);
-    e.slope_a = a1 - a0;
-    e.nslope_b = b0 - b1;
-    return e;
+    erow[i] = make_uint4(__float_as_uint(ma), __float_as_uint(mb), __float_as_uint(sa), __float_as_uint(sb));
+}
+__device__ __forceinline__ void store_entry(uint4* erow, int pitch, int i, double ma, double mb, double sa, double sb)
+{
+    reinterpret_cast<double2*>(erow)[i] = make_double2(ma, mb);
+    reinterpret_cast<double2*>(erow)[pitch + i] = make_double2(sa, sb);
+}
+
+template <typename T>
+__device__ __forceinline__ void store_entries(const T* yz, uint4* erow, int pitch, int tid, int nthr)
+{
+    for (int i = tid; i < pitch; i += nthr) {
+        const T a0 = yz[i + 1], a1 = yz[i + 2];
+        const T b0 = yz[pitch - 1 - i], b1 = yz[pitch - i];
+        store_entry(erow, pitch, i, T(0.5) * (a0 + a1), T(0.5) * (b0 + b1), a1 - a0, b0 - b1);
+    }
 }
 
 template <typename T, int R>
 __global__ void __launch_bounds__(512)
-filter_kernel(const T* __restrict__ P, T* __restrict__ Q, BpEntry<T>* __restrict__ E,
+filter_kernel(const T* __restrict__ P, T* __restrict__ Q, uint4* __restrict__ E,
               const T* __restrict__ G_gmem, const T* __restrict__ rho, FilterParams prm, T inv_d)
 {
     extern __shared__ __align__(16) unsigned char filt_smem_raw[];
@@ -157,30 +168,37 @@ filter_kernel(const T* __restrict__ P, T* __restrict__ Q, BpEntry<T>* __restrict
     __syncthreads();
 
     // ---- stores: plain row and/or interleaved entries, coalesced ----
-    // X0/X1 are dead now: reuse them as the row in natural order.
-    T* Yn = X0;
-    for (int n = tid; n < D; n += nthr) Yn[n] = Y[(n & 1) * prm.n_ob * blk + (n >> 1)];
+    // yz[k] = Q~[k - 1 - guard]: the row in natural order with zero guards (see store_entries)
+    T* yz = part + (size_t)prm.n_sb * y_pitch;
+    for (int k = tid; k < prm.ent_pitch + 2; k += nthr) {
+        const int n = k - 1 - prm.ent_guard;
+        yz[k] = (n >= 0 && n < D) ? Y[(n & 1) * prm.n_ob * blk + (n >> 1)] : T(0);
+    }
     __syncthreads();
     if (Q) {
         T* q = Q + (size_t)row * D;
-        for (int n = tid; n < D; n += nthr) q[n] = Yn[n];
+        const T* yn = yz + 1 + prm.ent_guard;
+        for (int n = tid; n < D; n += nthr) q[n] = yn[n];
     }
-    if (E) {
-        BpEntry<T>* e = E + (size_t)row * prm.ent_pitch;
-        for (int i = tid; i < prm.ent_pitch; i += nthr) e[i] = make_entry<T>(Yn, D, i - prm.ent_guard);
-    }
+    if (E) store_entries<T>(yz, E + (size_t)row * EntryPlanes<T>::value * prm.ent_pitch, prm.ent_pitch, tid, nthr);
 }
 
 // Plain filtered rows -> interleaved entries (fbp_backproject's first step); same arithmetic
 // as the filter epilogue, so fbp_reconstruct == fbp_backproject(fbp_filter) bit for bit.
 template <typename T>
 __global__ void __launch_bounds__(256)
-entries_kernel(const T* __restrict__ Q, BpEntry<T>* __restrict__ E, int n_det, int ent_pitch, int ent_guard)
+entries_kernel(const T* __restrict__ Q, uint4* __restrict__ E, int n_det, int ent_pitch, int ent_guard)
 {
+    extern __shared__ __align__(16) unsigned char ent_smem_raw[];
+    T* yz = reinterpret_cast<T*>(ent_smem_raw);
     const int row = blockIdx.x;
     const T* q = Q + (size_t)row * n_det;
-    BpEntry<T>* e = E + (size_t)row * ent_pitch;
-    for (int i = threadIdx.x; i < ent_pitch; i += blockDim.x) e[i] = make_entry<T>(q, n_det, i - ent_guard);
+    for (int k = threadIdx.x; k < ent_pitch + 2; k += blockDim.x) {
+        const int n = k - 1 - ent_guard;
+        yz[k] = (n >= 0 && n < n_det) ? q[n] : T(0);
+    }
+    __syncthreads();
+    store_entries<T>(yz, E + (size_t)row * EntryPlanes<T>::value * ent_pitch, ent_pitch, threadIdx.x, blockDim.x);
 }
 
 }  // namespace fbp
