@@ -17,6 +17,7 @@
 
 #include "fbp_backproject.cuh"
 #include "fbp_filter.cuh"
+#include "fbp_filter2.cuh"
 
 namespace {
 
@@ -60,6 +61,14 @@ struct fbp_plan {
     int f_r = 9, f_threads = 0, f_smem = 0, f_tab_len = 0;
     fbp::FilterParams fp{};
 
+    // paired-parity filter (fbp_filter2.cuh); filter_v = 1 selects the older one-parity kernel
+    int filter_v = 2;
+    int f2_r = 6, f2_threads = 0, f2_smem = 0, f2_grid_cap = 0;
+    fbp::Filter2Params f2{};
+    void* d_u = nullptr;        // [2][tab_len] dtype: UA | UB, U[j] = g[a_tot - 1 - j]
+    void* d_rho2 = nullptr;     // [D] dtype: conditioning term of the paired-parity filter
+
+    bool use_pdl = true;
     bool profiling = false;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     bool ran_filter = false, ran_bp = false;
@@ -147,6 +156,55 @@ void configure_filter(fbp_plan* p)
     p->f_smem = (int)(words * p->esize + 16);
 }
 
+// Paired-parity filter: R output pairs per thread (R = 2 mod 4), warps = n_ob output blocks x SB
+// input slices, persistent CTAs.
+void configure_filter2(fbp_plan* p)
+{
+    const int D = p->D;
+    const int na = (D + 1) / 2;                        // output pairs = input pairs
+    static const int cand[] = {6, 10, 14};
+    const int forced = env_int("FBP_FILTER_R", 0);
+    int best_r = 6;
+    double best = -1.0;
+    for (int R : cand) {
+        const int n_ob = (na + 32 * R - 1) / (32 * R);
+        if (n_ob > 16) continue;
+        if (p->dtype == FBP_F64 && R > 6) continue;   // 4R fp64 registers of accumulators and taps: R = 10 spills
+        const double util = (double)na / ((double)n_ob * 32 * R);
+        const double score = util * (2.0 * R) / (2.0 * R + 2.5);
+        if (forced == R) { best_r = R; best = 1e9; }
+        if (score > best) { best = score; best_r = R; }
+    }
+    const int R = best_r;
+    p->f2_r = R;
+    fbp::Filter2Params& f = p->f2;
+    f.n_det = D;
+    f.n_ob = (na + 32 * R - 1) / (32 * R);
+    f.a_tot = f.n_ob * 32 * R;
+    f.n_chunks = (na + R - 1) / R;
+    f.b_pad = f.n_chunks * R;
+    int sb = env_int("FBP_FILTER_SB", 0);
+    if (sb <= 0) {
+        // warps per CTA: few when rows are plentiful (less reduction work per row), more when one launch
+        // has only a few rows per SM or a row needs many output blocks (measured on B200)
+        const double rows_per_sm = (double)p->max_batch * p->K / kNumSm;
+        const int target = rows_per_sm >= 64.0 ? 4 : (f.n_ob >= 4 ? 16 : 8);
+        sb = (target + f.n_ob / 2) / f.n_ob;
+        if (sb < 1) sb = 1;
+    }
+    if (sb > 8) sb = 8;
+    if (sb > f.n_chunks) sb = f.n_chunks;
+    while (sb > 1 && f.n_ob * sb > 16) --sb;
+    if (sb < 1) sb = 1;
+    f.n_sb = sb;
+    f.tab_len = round_up(f.a_tot + f.b_pad + 2, 4);
+    f.ent_pitch = p->bp.ent_pitch; f.ent_guard = p->bp.ent_guard;
+    p->f2_threads = f.n_ob * sb * 32;
+    const size_t elems = 2 * (size_t)f.tab_len + 4 * (size_t)f.b_pad + (size_t)f.n_ob * 32 +
+                         (size_t)sb * 2 * f.a_tot + (size_t)(f.ent_pitch + 2) + (size_t)D;
+    p->f2_smem = (int)(elems * p->esize + 16);
+}
+
 // ---- back-projection launch configuration ------------------------------------------
 // (R, WY, WA) instantiations of backproject_kernel, see launch_bp
 constexpr int kNumBpVariants = 11;
@@ -228,6 +286,19 @@ void configure_bp(fbp_plan* p, const std::vector<double>& cs)
     const size_t red_bytes = (size_t)(kBpVariants[v][2] - 1) * 2 * p->bp_r * (32 * kBpVariants[v][1]) * p->esize;
     if (seg_bytes < red_bytes) seg_bytes = red_bytes;          // in-CTA reduction reuses the stages
     p->bp_smem = (int)(64 + fbp::kBpStages * rec * chunk + 128 + seg_bytes);
+    // A small launch (c CTAs per SM on average, c <= 5) is placed evenly only if no SM can hold more
+    // than c of its CTAs: with programmatic dependent launch the CTAs arrive while the filter is
+    // still draining and would otherwise pile up (up to 6 per SM) on the SMs that free up first.
+    // Padding the dynamic shared memory so that c + 1 CTAs do not fit caps the residency at c.
+    {
+        const long ctas = tiles * S;
+        const int cps = (int)((ctas + kNumSm - 1) / kNumSm);
+        const int smem_sm = 228 * 1024, reserve = 1024;
+        if (cps >= 1 && cps <= 5 && env_int("FBP_BP_EVEN", 1)) {
+            const int want = smem_sm / (cps + 1) - reserve + 256;
+            if (want > p->bp_smem && (long)cps * (want + reserve) <= smem_sm) p->bp_smem = want;
+        }
+    }
 
     fbp::BpParams& b = p->bp;
     b.n_angles = K; b.n_det = p->D; b.image_n = N;
@@ -275,6 +346,38 @@ cudaError_t launch_filter(const fbp_plan* p, const void* sino, void* filt, void*
     }
 }
 
+template <typename T, int R>
+cudaError_t launch_filter2_r(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st)
+{
+    fbp::Filter2Params f = p->f2;
+    f.n_rows = batch * p->K;
+    auto kern = fbp::filter2_kernel<T, R>;
+    if (p->f2_grid_cap == 0) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, p->f2_smem);
+        if (e != cudaSuccess) return e;
+        int per_sm = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, p->f2_threads, p->f2_smem);
+        if (e != cudaSuccess) return e;
+        if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+        p->f2_grid_cap = per_sm * kNumSm;
+    }
+    const int grid = f.n_rows < p->f2_grid_cap ? f.n_rows : p->f2_grid_cap;
+    kern<<<grid, p->f2_threads, p->f2_smem, st>>>(static_cast<const T*>(sino), static_cast<T*>(filt),
+                                                  static_cast<uint4*>(ent), static_cast<const T*>(p->d_u),
+                                                  static_cast<const T*>(p->d_rho2), f, (T)(1.0 / p->d));
+    return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t launch_filter2(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st)
+{
+    switch (p->f2_r) {
+        case 6: return launch_filter2_r<T, 6>(p, sino, filt, ent, batch, st);
+        case 10: return launch_filter2_r<T, 10>(p, sino, filt, ent, batch, st);
+        default: return launch_filter2_r<T, 14>(p, sino, filt, ent, batch, st);
+    }
+}
+
 template <typename T>
 cudaError_t launch_entries(const fbp_plan* p, const void* filt, int batch, cudaStream_t st)
 {
@@ -293,11 +396,21 @@ cudaError_t launch_bp_v(const fbp_plan* p, void* image, int batch, cudaStream_t 
     auto kern = fbp::backproject_kernel<T, R, WY, WA>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, p->bp_smem);
     if (e != cudaSuccess) return e;
-    dim3 grid(p->bp.tiles_x * p->bp.tiles_y, p->bp_splits, batch);
-    kern<<<grid, 32 * (WY * WA + 1), p->bp_smem, st>>>(static_cast<const uint4*>(p->d_ent), static_cast<T*>(image),
-                                            static_cast<const double2*>(p->d_cs2), static_cast<T*>(p->d_part),
-                                            p->d_tickets, p->bp);
-    return cudaGetLastError();
+    // programmatic dependent launch: the CTAs may become resident and run their prologue while the
+    // kernel that writes the entries (filter / entries_kernel) drains; the producer warp executes
+    // griddepcontrol.wait before its first read of the entries
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(p->bp.tiles_x * p->bp.tiles_y, p->bp_splits, batch);
+    cfg.blockDim = dim3(32 * (WY * WA + 1));
+    cfg.dynamicSmemBytes = (size_t)p->bp_smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = p->use_pdl ? 1 : 0;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<const uint4*>(p->d_ent), static_cast<T*>(image),
+                              static_cast<const double2*>(p->d_cs2), static_cast<T*>(p->d_part), p->d_tickets, p->bp);
 }
 
 // back-projection of the plan's entry buffer into `image`
@@ -333,8 +446,13 @@ fbp_status check_call(fbp_plan* p, const void* a, const void* b, int batch)
 fbp_status run_filter(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st)
 {
     if (p->profiling) FBP_CUDA(p, cudaEventRecord(p->ev[0], st));
-    cudaError_t e = p->dtype == FBP_F32 ? launch_filter<float>(p, sino, filt, ent, batch, st)
-                                        : launch_filter<double>(p, sino, filt, ent, batch, st);
+    cudaError_t e;
+    if (p->filter_v == 2)
+        e = p->dtype == FBP_F32 ? launch_filter2<float>(p, sino, filt, ent, batch, st)
+                                : launch_filter2<double>(p, sino, filt, ent, batch, st);
+    else
+        e = p->dtype == FBP_F32 ? launch_filter<float>(p, sino, filt, ent, batch, st)
+                                : launch_filter<double>(p, sino, filt, ent, batch, st);
     if (e != cudaSuccess) return cuda_fail(p, e, "filter launch");
     if (p->profiling) FBP_CUDA(p, cudaEventRecord(p->ev[1], st));
     p->ran_filter = true;
@@ -410,10 +528,14 @@ fbp_status fbp_create(fbp_plan** out, int n_angles, int n_det, const double* ang
     }
     configure_bp(p, cs);
     configure_filter(p);   // after configure_bp: needs the entry pitch
+    configure_filter2(p);
+    p->filter_v = env_int("FBP_FILTER_V", 2) == 1 ? 1 : 2;
+    p->use_pdl = env_int("FBP_PDL", 1) != 0;
 
     auto bail = [&](fbp_status st) { std::string m = p->err; fbp_destroy(p); g_create_error = m; return st; };
-    if (p->f_threads > 512) { p->err = "n_det too large for the row filter (more than 512 threads per row)"; return bail(FBP_EUNSUPPORTED); }
-    if (p->f_smem > 220 * 1024) { p->err = "n_det too large for the shared-memory row filter"; return bail(FBP_EUNSUPPORTED); }
+    if (p->filter_v == 2 && (p->f2_threads > 512 || p->f2_smem > 220 * 1024)) p->filter_v = 1;
+    if (p->filter_v == 1 && p->f_threads > 512) { p->err = "n_det too large for the row filter (more than 512 threads per row)"; return bail(FBP_EUNSUPPORTED); }
+    if (p->filter_v == 1 && p->f_smem > 220 * 1024) { p->err = "n_det too large for the shared-memory row filter"; return bail(FBP_EUNSUPPORTED); }
     if (p->bp_smem > 220 * 1024) { p->err = "pixel_size/det_spacing too large for the staged segment"; return bail(FBP_EUNSUPPORTED); }
 
     DeviceGuard guard(device);
@@ -442,6 +564,31 @@ fbp_status fbp_create(fbp_plan** out, int n_angles, int n_det, const double* ang
         for (double t : terms) ssum += t;
         rho64[n] = 0.25 - ssum;
     }
+    // paired-parity filter tables: U[j] = g[a_tot - 1 - j] as UA | UB (UB[j] = U[j+1]); rho2[n] = 1/4 +
+    // sum_{b < b_pad} g[a - b - (1 - p)], n = 2a + p  (constant-row response, smallest terms first)
+    const int tl2 = p->f2.tab_len;
+    std::vector<double> u64(2 * (size_t)tl2), rho2_64(n_det);
+    auto gq = [](long long q) { const double m = 2.0 * (double)q + 1.0; return -1.0 / (kPi * kPi * m * m); };
+    for (int j = 0; j < tl2; ++j) {
+        u64[j] = gq((long long)p->f2.a_tot - 1 - j);
+        u64[tl2 + j] = gq((long long)p->f2.a_tot - 2 - j);
+    }
+    for (int n = 0; n < n_det; ++n) {
+        const int par = n & 1, a = n >> 1;
+        std::vector<double> terms(p->f2.b_pad);
+        for (int b = 0; b < p->f2.b_pad; ++b) terms[b] = -gq((long long)a - b - (1 - par));
+        std::sort(terms.begin(), terms.end());
+        double ssum = 0.0;
+        for (double t : terms) ssum += t;
+        rho2_64[n] = 0.25 - ssum;
+    }
+    std::vector<float> u32, rho2_32;
+    const void* usrc = u64.data();
+    const void* r2src = rho2_64.data();
+    if (dtype == FBP_F32) {
+        u32.assign(u64.begin(), u64.end()); usrc = u32.data();
+        rho2_32.assign(rho2_64.begin(), rho2_64.end()); r2src = rho2_32.data();
+    }
     std::vector<float> g32, rho32;
     const void* gsrc = g64.data();
     const void* rsrc = rho64.data();
@@ -461,6 +608,10 @@ fbp_status fbp_create(fbp_plan** out, int n_angles, int n_det, const double* ang
     FBP_TRY(cudaMemcpy(p->d_taps, gsrc, p->esize * (size_t)tl, cudaMemcpyHostToDevice));
     FBP_TRY(cudaMalloc(&p->d_rho, p->esize * (size_t)n_det));
     FBP_TRY(cudaMemcpy(p->d_rho, rsrc, p->esize * (size_t)n_det, cudaMemcpyHostToDevice));
+    FBP_TRY(cudaMalloc(&p->d_u, p->esize * 2 * (size_t)tl2));
+    FBP_TRY(cudaMemcpy(p->d_u, usrc, p->esize * 2 * (size_t)tl2, cudaMemcpyHostToDevice));
+    FBP_TRY(cudaMalloc(&p->d_rho2, p->esize * (size_t)n_det));
+    FBP_TRY(cudaMemcpy(p->d_rho2, r2src, p->esize * (size_t)n_det, cudaMemcpyHostToDevice));
     FBP_TRY(cudaMalloc(&p->d_ent, 4 * p->esize * (size_t)max_batch * n_angles * p->bp.ent_pitch));
     if (p->bp_splits > 1) {
         const size_t nt = (size_t)max_batch * p->bp.tiles_x * p->bp.tiles_y;
@@ -480,7 +631,7 @@ void fbp_destroy(fbp_plan* p)
     {
         DeviceGuard guard(p->device);
         cudaFree(p->d_cs2); cudaFree(p->d_taps); cudaFree(p->d_rho); cudaFree(p->d_ent); cudaFree(p->d_part); cudaFree(p->d_tickets);
-        cudaFree(p->d_hsino); cudaFree(p->d_himg);
+        cudaFree(p->d_hsino); cudaFree(p->d_himg); cudaFree(p->d_u); cudaFree(p->d_rho2);
         for (int i = 0; i < 4; ++i) if (p->ev[i]) cudaEventDestroy(p->ev[i]);
         cudaGetLastError();
     }
@@ -550,7 +701,8 @@ int fbp_plan_info(const fbp_plan* p, int* out, int n)
     if (!p) return 0;
     const int v[14] = {p->bp_tw, p->bp_th, p->bp_r, p->bp_splits, p->bp_chunk, p->bp_seg,
                        p->bp.tiles_x * p->bp.tiles_y * p->bp_splits, p->bp_threads, p->bp_smem,
-                       p->f_r, p->f_threads, p->fp.n_sb, p->f_smem,
+                       p->filter_v == 2 ? 2 * p->f2_r : p->f_r, p->filter_v == 2 ? p->f2_threads : p->f_threads,
+                       p->filter_v == 2 ? p->f2.n_sb : p->fp.n_sb, p->filter_v == 2 ? p->f2_smem : p->f_smem,
                        2};
     if (out) for (int i = 0; i < n && i < 14; ++i) out[i] = v[i];
     return 14;

@@ -201,6 +201,10 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
         fence_mbar_init();
     }
     __syncthreads();
+    // programmatic dependent launch: everything above overlapped the tail of the kernel that writes
+    // E.  Every thread blocks here (consumers would otherwise spin on their mbarriers and take issue
+    // slots from that kernel); a no-op when launched without the attribute.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
 
     PairAcc<T> acc[R];
 #pragma unroll

@@ -191,6 +191,7 @@ entries_kernel(const T* __restrict__ Q, uint4* __restrict__ E, int n_det, int en
 {
     extern __shared__ __align__(16) unsigned char ent_smem_raw[];
     T* yz = reinterpret_cast<T*>(ent_smem_raw);
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the back-projector may start its prologue
     const int row = blockIdx.x;
     const T* q = Q + (size_t)row * n_det;
     for (int k = threadIdx.x; k < ent_pitch + 2; k += blockDim.x) {
