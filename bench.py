@@ -333,6 +333,8 @@ def main():
                        plan=r["info"]),
         "slices_per_s": cfg.batch * world / (r["ms_step"] * 1e-3),
         "kernels": {"filter_ms": r["f_ms"], "backproject_ms": r["b_ms"], "backproject_gupdates_per_s": bp_gups,
+                    "backproject_smem_operand_tbs": bp_gups * 1e9 * 2 * r["esize"] / 1e12,
+                    "backproject_frac_of_smem_ceiling": bp_gups * 1e9 * 2 * r["esize"] / (SM_COUNT * 128 * sm_max_mhz * 1e6),
                     "filter_hbm_gbs": filt_bytes / (r["f_ms"] * 1e-3) / 1e9,
                     "filter_hbm_frac_of_%s" % peaks_src: filt_bytes / (r["f_ms"] * 1e-3) / 1e9 / float(peaks["hbm_gbs"]),
                     "filter_tfma_per_s": filt_fma / (r["f_ms"] * 1e-3) / 1e12,

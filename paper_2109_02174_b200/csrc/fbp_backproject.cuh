@@ -157,7 +157,10 @@ template <> struct PairAcc<double> {
 #ifndef FBP_BP_REGCAP
 #define FBP_BP_REGCAP (sizeof(T) == 4 ? 64 : 96)
 #endif
-constexpr int kBpStages = 3;
+#ifndef FBP_BP_STAGES
+#define FBP_BP_STAGES 3
+#endif
+constexpr int kBpStages = FBP_BP_STAGES;
 
 template <typename T, int R, int WY, int WA>
 __global__ void __launch_bounds__(32 * (WY * WA + 1), 65536 / (FBP_BP_REGCAP * 32 * (WY * WA + 1)))
