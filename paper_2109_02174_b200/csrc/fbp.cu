@@ -69,6 +69,11 @@ struct fbp_plan {
     void* d_rho2 = nullptr;     // [D] dtype: conditioning term of the paired-parity filter
 
     bool use_pdl = true;
+    // batch pipeline (run_pipelined): filter of slice group g+1 overlaps back-projection of group g
+    static constexpr int kMaxGroups = 16;
+    int pipe_min_batch = 8, pipe_group = 0;
+    cudaStream_t st_f = nullptr, st_b[2] = {nullptr, nullptr};
+    cudaEvent_t ev_fork = nullptr, ev_f[kMaxGroups] = {}, ev_b[2] = {nullptr, nullptr};
     bool profiling = false;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     bool ran_filter = false, ran_bp = false;
@@ -399,7 +404,7 @@ cudaError_t launch_entries(const fbp_plan* p, const void* filt, int batch, cudaS
 }
 
 template <typename T, int R, int WY, int WA>
-cudaError_t launch_bp_v(const fbp_plan* p, void* image, int batch, cudaStream_t st)
+cudaError_t launch_bp_v(const fbp_plan* p, void* image, int batch, cudaStream_t st, int slice0)
 {
     auto kern = fbp::backproject_kernel<T, R, WY, WA>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, p->bp_smem);
@@ -417,26 +422,29 @@ cudaError_t launch_bp_v(const fbp_plan* p, void* image, int batch, cudaStream_t 
     attr[0].val.programmaticStreamSerializationAllowed = p->use_pdl ? 1 : 0;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, kern, static_cast<const uint4*>(p->d_ent), static_cast<T*>(image),
+    // slice0: first slice of this launch within the plan's entry buffer (`image` already points at it)
+    const uint4* ent = static_cast<const uint4*>(p->d_ent) +
+                       (size_t)slice0 * p->K * fbp::EntryPlanes<T>::value * p->bp.ent_pitch;
+    return cudaLaunchKernelEx(&cfg, kern, ent, static_cast<T*>(image),
                               static_cast<const double2*>(p->d_cs2), static_cast<T*>(p->d_part), p->d_tickets, p->bp);
 }
 
 // back-projection of the plan's entry buffer into `image`
 template <typename T>
-cudaError_t launch_bp(const fbp_plan* p, void* image, int batch, cudaStream_t st)
+cudaError_t launch_bp(const fbp_plan* p, void* image, int batch, cudaStream_t st, int slice0 = 0)
 {
     switch (p->bp_variant) {
-        case 0: return launch_bp_v<T, 8, 4, 1>(p, image, batch, st);
-        case 1: return launch_bp_v<T, 4, 4, 1>(p, image, batch, st);
-        case 2: return launch_bp_v<T, 4, 1, 4>(p, image, batch, st);
-        case 3: return launch_bp_v<T, 5, 1, 4>(p, image, batch, st);
-        case 4: return launch_bp_v<T, 6, 1, 4>(p, image, batch, st);
-        case 5: return launch_bp_v<T, 7, 1, 4>(p, image, batch, st);
-        case 6: return launch_bp_v<T, 8, 1, 4>(p, image, batch, st);
-        case 7: return launch_bp_v<T, 4, 1, 8>(p, image, batch, st);
-        case 8: return launch_bp_v<T, 6, 1, 8>(p, image, batch, st);
-        case 9: return launch_bp_v<T, 7, 1, 8>(p, image, batch, st);
-        default: return launch_bp_v<T, 8, 1, 8>(p, image, batch, st);
+        case 0: return launch_bp_v<T, 8, 4, 1>(p, image, batch, st, slice0);
+        case 1: return launch_bp_v<T, 4, 4, 1>(p, image, batch, st, slice0);
+        case 2: return launch_bp_v<T, 4, 1, 4>(p, image, batch, st, slice0);
+        case 3: return launch_bp_v<T, 5, 1, 4>(p, image, batch, st, slice0);
+        case 4: return launch_bp_v<T, 6, 1, 4>(p, image, batch, st, slice0);
+        case 5: return launch_bp_v<T, 7, 1, 4>(p, image, batch, st, slice0);
+        case 6: return launch_bp_v<T, 8, 1, 4>(p, image, batch, st, slice0);
+        case 7: return launch_bp_v<T, 4, 1, 8>(p, image, batch, st, slice0);
+        case 8: return launch_bp_v<T, 6, 1, 8>(p, image, batch, st, slice0);
+        case 9: return launch_bp_v<T, 7, 1, 8>(p, image, batch, st, slice0);
+        default: return launch_bp_v<T, 8, 1, 8>(p, image, batch, st, slice0);
     }
 }
 
@@ -482,6 +490,51 @@ fbp_status run_bp(fbp_plan* p, const void* filt, void* image, int batch, cudaStr
     if (p->profiling) FBP_CUDA(p, cudaEventRecord(p->ev[3], st));
     p->ran_bp = true;
     return FBP_OK;
+}
+
+// fbp_reconstruct for a stack of slices: the filter is FMA-pipe bound and the back-projector
+// shared-memory bound, so they run well side by side.  The batch is cut into groups; group g+1 is
+// filtered on a plan-owned high-priority stream while group g is back-projected on one of two other
+// plan-owned streams (two, so that the tail of one launch overlaps the head of the next).  The
+// caller's stream forks into them and joins at the end: still enqueue-only, no host wait.  Same
+// kernels on the same data as the sequential path, hence the same bytes.
+fbp_status run_pipelined(fbp_plan* p, const void* sino, void* image, int batch, cudaStream_t s)
+{
+    int group = p->pipe_group > 0 ? p->pipe_group : (batch + 3) / 4;   // 4 groups measured best at 64 slices
+    const int min_group = (batch + fbp_plan::kMaxGroups - 1) / fbp_plan::kMaxGroups;
+    if (group < min_group) group = min_group;
+    const int n_groups = (batch + group - 1) / group;
+    const size_t sino_slice = p->esize * (size_t)p->K * p->D, img_slice = p->esize * (size_t)p->N * p->N;
+    const size_t ent_slice = 4 * p->esize * (size_t)p->K * p->bp.ent_pitch;
+    FBP_CUDA(p, cudaEventRecord(p->ev_fork, s));
+    FBP_CUDA(p, cudaStreamWaitEvent(p->st_f, p->ev_fork, 0));
+    FBP_CUDA(p, cudaStreamWaitEvent(p->st_b[0], p->ev_fork, 0));
+    FBP_CUDA(p, cudaStreamWaitEvent(p->st_b[1], p->ev_fork, 0));
+    for (int g = 0; g < n_groups; ++g) {
+        const int g0 = g * group, nb = batch - g0 < group ? batch - g0 : group;
+        const char* sg = static_cast<const char*>(sino) + (size_t)g0 * sino_slice;
+        char* eg = static_cast<char*>(p->d_ent) + (size_t)g0 * ent_slice;
+        cudaError_t e = p->dtype == FBP_F32 ? launch_filter2<float>(p, sg, nullptr, eg, nb, p->st_f)
+                                            : launch_filter2<double>(p, sg, nullptr, eg, nb, p->st_f);
+        if (e != cudaSuccess) return cuda_fail(p, e, "filter launch");
+        FBP_CUDA(p, cudaEventRecord(p->ev_f[g], p->st_f));
+        cudaStream_t sb = p->st_b[g & 1];
+        FBP_CUDA(p, cudaStreamWaitEvent(sb, p->ev_f[g], 0));
+        char* ig = static_cast<char*>(image) + (size_t)g0 * img_slice;
+        e = p->dtype == FBP_F32 ? launch_bp<float>(p, ig, nb, sb, g0) : launch_bp<double>(p, ig, nb, sb, g0);
+        if (e != cudaSuccess) return cuda_fail(p, e, "back-projection launch");
+    }
+    for (int i = 0; i < 2; ++i) {
+        FBP_CUDA(p, cudaEventRecord(p->ev_b[i], p->st_b[i]));
+        FBP_CUDA(p, cudaStreamWaitEvent(s, p->ev_b[i], 0));
+    }
+    p->ran_filter = p->ran_bp = false;
+    return FBP_OK;
+}
+
+bool use_pipeline(const fbp_plan* p, int batch)
+{
+    return p->st_f && !p->profiling && p->filter_v == 2 && p->bp_splits == 1 && batch >= p->pipe_min_batch;
 }
 
 }  // namespace
@@ -628,6 +681,17 @@ fbp_status fbp_create(fbp_plan** out, int n_angles, int n_det, const double* ang
         FBP_TRY(cudaMemset(p->d_tickets, 0, sizeof(int) * nt));
     }
     for (int i = 0; i < 4; ++i) FBP_TRY(cudaEventCreate(&p->ev[i]));
+    p->pipe_min_batch = env_int("FBP_PIPE_MIN_BATCH", 8);
+    p->pipe_group = env_int("FBP_PIPE_GROUP", 0);
+    if (env_int("FBP_PIPE", 1) && max_batch >= p->pipe_min_batch) {
+        int prio_lo = 0, prio_hi = 0;
+        FBP_TRY(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+        FBP_TRY(cudaStreamCreateWithPriority(&p->st_f, cudaStreamNonBlocking, prio_hi));
+        for (int i = 0; i < 2; ++i) FBP_TRY(cudaStreamCreateWithPriority(&p->st_b[i], cudaStreamNonBlocking, prio_lo));
+        FBP_TRY(cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming));
+        for (int i = 0; i < fbp_plan::kMaxGroups; ++i) FBP_TRY(cudaEventCreateWithFlags(&p->ev_f[i], cudaEventDisableTiming));
+        for (int i = 0; i < 2; ++i) FBP_TRY(cudaEventCreateWithFlags(&p->ev_b[i], cudaEventDisableTiming));
+    }
 #undef FBP_TRY
     *out = p;
     return FBP_OK;
@@ -641,6 +705,11 @@ void fbp_destroy(fbp_plan* p)
         cudaFree(p->d_cs2); cudaFree(p->d_taps); cudaFree(p->d_rho); cudaFree(p->d_ent); cudaFree(p->d_part); cudaFree(p->d_tickets);
         cudaFree(p->d_hsino); cudaFree(p->d_himg); cudaFree(p->d_u); cudaFree(p->d_rho2);
         for (int i = 0; i < 4; ++i) if (p->ev[i]) cudaEventDestroy(p->ev[i]);
+        if (p->st_f) { cudaStreamSynchronize(p->st_f); cudaStreamDestroy(p->st_f); }
+        for (int i = 0; i < 2; ++i) if (p->st_b[i]) { cudaStreamSynchronize(p->st_b[i]); cudaStreamDestroy(p->st_b[i]); }
+        if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+        for (int i = 0; i < fbp_plan::kMaxGroups; ++i) if (p->ev_f[i]) cudaEventDestroy(p->ev_f[i]);
+        for (int i = 0; i < 2; ++i) if (p->ev_b[i]) cudaEventDestroy(p->ev_b[i]);
         cudaGetLastError();
     }
     delete p;
@@ -678,6 +747,7 @@ fbp_status fbp_reconstruct(fbp_plan* p, const void* d_sino, void* d_image, int b
     DeviceGuard guard(p->device);
     p->ran_filter = p->ran_bp = false;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (use_pipeline(p, batch)) return run_pipelined(p, d_sino, d_image, batch, s);
     st = run_filter(p, d_sino, nullptr, p->d_ent, batch, s);
     if (st != FBP_OK) return st;
     return run_bp(p, nullptr, d_image, batch, s);
@@ -695,9 +765,14 @@ fbp_status fbp_reconstruct_host(fbp_plan* p, const void* h_sino, void* h_image, 
     if (!p->d_himg) FBP_CUDA(p, cudaMalloc(&p->d_himg, img_bytes * p->max_batch));
     FBP_CUDA(p, cudaMemcpyAsync(p->d_hsino, h_sino, sino_bytes * batch, cudaMemcpyHostToDevice, s));
     p->ran_filter = p->ran_bp = false;
-    fbp_status st = run_filter(p, p->d_hsino, nullptr, p->d_ent, batch, s);
-    if (st != FBP_OK) return st;
-    st = run_bp(p, nullptr, p->d_himg, batch, s);
+    fbp_status st;
+    if (use_pipeline(p, batch)) {
+        st = run_pipelined(p, p->d_hsino, p->d_himg, batch, s);
+    } else {
+        st = run_filter(p, p->d_hsino, nullptr, p->d_ent, batch, s);
+        if (st != FBP_OK) return st;
+        st = run_bp(p, nullptr, p->d_himg, batch, s);
+    }
     if (st != FBP_OK) return st;
     FBP_CUDA(p, cudaMemcpyAsync(h_image, p->d_himg, img_bytes * batch, cudaMemcpyDeviceToHost, s));
     FBP_CUDA(p, cudaStreamSynchronize(s));
