@@ -15,4 +15,9 @@ from .oracle import (  # noqa: F401
     backproject_pixels,
     forward_scatter,
     reconstruct,
+    WINDOWS,
+    window_taps,
+    filter_sinogram_window,
+    backproject_weighted,
+    metrics,
 )

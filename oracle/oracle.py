@@ -14,6 +14,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "fbp_oracle.c")
+_SRC_EXT = os.path.join(_HERE, "fbp_oracle_ext.c")
 _LIB = os.path.join(_HERE, "libfbp_oracle.so")
 _lock = threading.Lock()
 _lib = None
@@ -25,10 +26,11 @@ _ip = ctypes.POINTER(ctypes.c_int)
 def build(force: bool = False) -> str:
     """Compile the oracle if the shared object is missing or older than its source."""
     with _lock:
-        stale = force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC)
+        stale = (force or not os.path.exists(_LIB)
+                 or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_EXT)))
         if stale:
             tmp = _LIB + ".tmp.%d" % os.getpid()
-            cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-o", tmp, _SRC, "-lm"]
+            cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-o", tmp, _SRC, _SRC_EXT, "-lm"]
             subprocess.run(cmd, check=True)
             os.replace(tmp, _LIB)
     return _LIB
@@ -55,6 +57,17 @@ def _load():
         lib.fbp_oracle_reconstruct.argtypes = [_dp, _dp, _dp, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                                _dp, ctypes.c_double, ctypes.c_int, ctypes.c_double,
                                                ctypes.c_int]
+        lib.fbp_oracle_window_taps.argtypes = [ctypes.c_int, ctypes.c_int, _dp]
+        lib.fbp_oracle_window_taps.restype = None
+        lib.fbp_oracle_filter_window.argtypes = [_dp, _dp, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                                 ctypes.c_double, ctypes.c_int, ctypes.c_int]
+        lib.fbp_oracle_filter_window.restype = None
+        lib.fbp_oracle_backproject_weighted.argtypes = [_dp, _dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp, _dp,
+                                                        ctypes.c_double, ctypes.c_int, ctypes.c_double, ctypes.c_int]
+        lib.fbp_oracle_backproject_weighted.restype = None
+        lib.fbp_oracle_metrics.argtypes = [_dp, _dp, ctypes.c_long, ctypes.c_double, ctypes.c_double,
+                                           ctypes.c_double, _dp]
+        lib.fbp_oracle_metrics.restype = None
         for fn in ("fbp_oracle_taps", "fbp_oracle_filter", "fbp_oracle_backproject",
                    "fbp_oracle_backproject_pixels", "fbp_oracle_filter_rows",
                    "fbp_oracle_forward_scatter", "fbp_oracle_reconstruct"):
@@ -174,3 +187,51 @@ def reconstruct(sino, angles, image_n: int, det_spacing: float = 1.0, pixel_size
     _load().fbp_oracle_reconstruct(_p(p3), _p(work), _p(f), b, k, d, _p(ang), float(det_spacing),
                                    int(image_n), pix, int(threads))
     return f[0] if p.ndim == 2 else f
+
+
+# ---- rows SURVEY.md 8(f) marks "next" (fbp_oracle_ext.c) --------------------------------------
+WINDOWS = {"ramlak": 0, "shepp-logan": 1, "cosine": 2, "hamming": 3, "hann": 4}
+
+
+def window_taps(n_det: int, window) -> np.ndarray:
+    """h_W[m], m = -(D-1)..D-1, of the apodised ramp |f| W(f) (W1 of fbp_oracle_ext.c)."""
+    lib = _load()
+    out = np.empty(2 * n_det - 1, dtype=np.float64)
+    lib.fbp_oracle_window_taps(int(n_det), int(WINDOWS.get(window, window)), _p(out))
+    return out
+
+
+def filter_sinogram_window(sino, window, det_spacing: float = 1.0, threads: int = 0) -> np.ndarray:
+    lib = _load()
+    p = _stack3(sino)
+    q = np.empty_like(p)
+    lib.fbp_oracle_filter_window(_p(p), _p(q), p.shape[0], p.shape[1], p.shape[2], float(det_spacing),
+                                 int(WINDOWS.get(window, window)), int(threads))
+    return q.reshape(np.shape(sino))
+
+
+def backproject_weighted(filtered, angles, weights, image_n: int, det_spacing: float = 1.0,
+                         pixel_size: float | None = None, threads: int = 0) -> np.ndarray:
+    """f = sum_i w_i lerp(Q_i, u_i): eq. 2 with caller-supplied per-angle weights (W2)."""
+    lib = _load()
+    q = _stack3(filtered)
+    ang, wts = _f64(angles), _f64(weights)
+    assert ang.shape == wts.shape == (q.shape[1],)
+    pix = float(det_spacing if pixel_size is None else pixel_size)
+    f = np.empty((q.shape[0], image_n, image_n), dtype=np.float64)
+    lib.fbp_oracle_backproject_weighted(_p(q), _p(f), q.shape[0], q.shape[1], q.shape[2], _p(ang), _p(wts),
+                                        float(det_spacing), int(image_n), pix, int(threads))
+    return f if np.ndim(filtered) == 3 else f[0]
+
+
+def metrics(x, y, max_val: float, c1: float | None = None, c2: float | None = None) -> dict:
+    """MSE, PSNR (eq. 3) and global-statistics SSIM (eq. 4) of one image pair (M1)."""
+    lib = _load()
+    a, b = _f64(x).ravel(), _f64(y).ravel()
+    assert a.shape == b.shape
+    c1 = (0.01 * max_val) ** 2 if c1 is None else c1
+    c2 = (0.03 * max_val) ** 2 if c2 is None else c2
+    out = np.empty(8, dtype=np.float64)
+    lib.fbp_oracle_metrics(_p(a), _p(b), a.size, float(max_val), float(c1), float(c2), _p(out))
+    keys = ("mse", "psnr", "ssim", "mu_x", "mu_y", "var_x", "var_y", "cov_xy")
+    return dict(zip(keys, (float(v) for v in out)))

@@ -1,0 +1,58 @@
+"""Small driver for `compute-sanitizer` (memcheck / racecheck / initcheck / synccheck):
+
+    compute-sanitizer --tool racecheck python -m paper_2109_02174_b200.selfcheck
+
+Runs every kernel family once on tiny geometries (both dtypes, angle splits on and off, the batch
+pipeline, the host path) and checks that repeated runs are bit-identical.  No oracle here: parity is
+the business of tests/; this only gives the sanitizer something to watch."""
+from __future__ import annotations
+
+import math
+import os
+import sys
+
+
+def main() -> int:
+    import numpy as np
+    import torch
+
+    import paper_2109_02174_b200 as pkg
+
+    pkg.load_library()
+    torch.cuda.set_device(0)
+    cases = [  # (N, K, D, batch, env)
+        (40, 24, 61, 1, {}),
+        (33, 10, 48, 2, {"FBP_BP_SPLITS": "3"}),
+        (64, 16, 91, 9, {}),                       # batch >= 8: pipelined path
+        (24, 8, 40, 1, {"FBP_FILTER_V": "1"}),
+    ]
+    for n, k, d, b, env in cases:
+        os.environ.update(env)
+        try:
+            ang = [i * math.pi / k for i in range(k)]
+            for dt, tdt in (("f32", torch.float32), ("f64", torch.float64)):
+                sino = torch.from_numpy(np.random.default_rng(n + k).standard_normal((b, k, d))).to(tdt).cuda()
+                with pkg.Plan(ang, d, n, dtype=dt, max_batch=b) as plan:
+                    first = plan.reconstruct(sino).clone()
+                    q = plan.filter(sino)
+                    two = plan.backproject(q)
+                    again = plan.reconstruct(sino)
+                    torch.cuda.synchronize()
+                    if not (torch.equal(first, again) and torch.equal(first, two)):
+                        print("MISMATCH", n, k, d, b, dt, env)
+                        return 1
+                    host_in = sino.cpu().pin_memory()
+                    host_out = torch.empty((b, n, n), dtype=tdt).pin_memory()
+                    pkg.fbp_reconstruct_host(plan.handle, host_in, host_out, b)
+                    if not torch.equal(host_out, first.cpu()):
+                        print("HOST MISMATCH", n, k, d, b, dt, env)
+                        return 1
+        finally:
+            for key in env:
+                os.environ.pop(key, None)
+    print("selfcheck ok")
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
