@@ -103,6 +103,22 @@ fbp_status fbp_reconstruct(fbp_plan *plan, const void *d_sino, void *d_image, in
 fbp_status fbp_reconstruct_host(fbp_plan *plan, const void *h_sino, void *h_image, int batch,
                                 void *cuda_stream);
 
+/*
+ * fbp_metrics -- the paper's image-similarity measures of one image pair:
+ *   PSNR = 20 log10(MAX / sqrt(MSE))                                        (eq. 3)
+ *   SSIM = (2 mu_x mu_y + C1)(2 s_xy + C2) / ((mu_x^2 + mu_y^2 + C1)(s_x^2 + s_y^2 + C2))
+ *                                                                            (eq. 4)
+ * with statistics over all n elements (the paper names no window): mu = mean, s^2 and s_xy =
+ * population variance and covariance.  d_x, d_y: DEVICE arrays of n elements of the plan's dtype
+ * (any shape, e.g. one image or a whole stack).  max_val = MAX > 0.  c1, c2 < 0 select the customary
+ * (0.01 MAX)^2 and (0.03 MAX)^2 (the paper does not state its constants).  d_out8: DEVICE array of
+ * 8 doubles, written on the stream: MSE, PSNR (+inf when MSE = 0), SSIM, mu_x, mu_y,
+ * s_x^2, s_y^2, s_xy.  fp64 sums in a fixed order: repeated calls give the same bits.  Enqueue-only;
+ * uses plan-owned scratch, so not concurrently with other calls on the same plan.
+ */
+fbp_status fbp_metrics(fbp_plan *plan, const void *d_x, const void *d_y, long long n, double max_val,
+                       double c1, double c2, double *d_out8, void *cuda_stream);
+
 /* fbp_destroy -- free the plan, its tables and scratch.  NULL-safe.  Synchronous. */
 void fbp_destroy(fbp_plan *plan);
 

@@ -10,7 +10,7 @@ from .binding import (  # noqa: F401
     EXPORTS, FBP_F32, FBP_F64, FBP_OK, FBP_EINVAL, FBP_ENOMEM, FBP_ECUDA, FBP_EUNSUPPORTED,
     FbpError, load_library,
     fbp_create, fbp_filter, fbp_backproject, fbp_reconstruct, fbp_reconstruct_host,
-    fbp_destroy, fbp_last_error, fbp_plan_info, fbp_set_profiling, fbp_get_kernel_ms,
+    fbp_destroy, fbp_last_error, fbp_plan_info, fbp_set_profiling, fbp_get_kernel_ms, fbp_metrics,
 )
 from .build import build  # noqa: F401
 
@@ -73,6 +73,18 @@ class Plan:
         out = self._empty(sino, (self.image_n, self.image_n)) if out is None else out
         fbp_reconstruct(self.handle, sino, out, b, stream)
         return out
+
+    def metrics(self, x, y, max_val, c1=-1.0, c2=-1.0, stream=None) -> dict:
+        """PSNR / SSIM (eq. 3, 4 of the paper) of two CUDA tensors of the plan dtype; one device-to-host read."""
+        import torch
+        if x.dtype != self.torch_dtype or y.dtype != self.torch_dtype or x.shape != y.shape:
+            raise ValueError("expected two tensors of the plan dtype and the same shape")
+        if not (x.is_cuda and y.is_cuda and x.is_contiguous() and y.is_contiguous()):
+            raise ValueError("expected contiguous CUDA tensors")
+        out = torch.empty(8, dtype=torch.float64, device=x.device)
+        fbp_metrics(self.handle, x, y, x.numel(), max_val, c1, c2, out, stream)
+        vals = out.cpu().tolist()
+        return dict(zip(("mse", "psnr", "ssim", "mu_x", "mu_y", "var_x", "var_y", "cov_xy"), vals))
 
     def close(self):
         if getattr(self, "handle", None):

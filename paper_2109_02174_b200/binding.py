@@ -18,6 +18,7 @@ STATUS_NAMES = {0: "FBP_OK", 1: "FBP_EINVAL", 2: "FBP_ENOMEM", 3: "FBP_ECUDA", 4
 EXPORTS = (
     "fbp_create", "fbp_filter", "fbp_backproject", "fbp_reconstruct", "fbp_reconstruct_host",
     "fbp_destroy", "fbp_last_error", "fbp_plan_info", "fbp_set_profiling", "fbp_get_kernel_ms",
+    "fbp_metrics",
 )
 
 PLAN_INFO_FIELDS = (
@@ -54,6 +55,8 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         fn = getattr(lib, name)
         fn.argtypes = [vp, vp, vp, ci, vp]
         fn.restype = ci
+    lib.fbp_metrics.argtypes = [vp, vp, vp, ctypes.c_longlong, cd, cd, cd, vp, vp]
+    lib.fbp_metrics.restype = ci
     lib.fbp_destroy.argtypes = [vp]
     lib.fbp_destroy.restype = None
     lib.fbp_last_error.argtypes = [vp]
@@ -159,3 +162,9 @@ def fbp_get_kernel_ms(plan):
     f, b = ctypes.c_float(), ctypes.c_float()
     _check(lib, plan, lib.fbp_get_kernel_ms(plan, ctypes.byref(f), ctypes.byref(b)))
     return f.value, b.value
+
+
+def fbp_metrics(plan, d_x, d_y, n, max_val, c1, c2, d_out8, stream=None):
+    lib = load_library()
+    _check(lib, plan, lib.fbp_metrics(plan, _ptr(d_x), _ptr(d_y), int(n), float(max_val), float(c1), float(c2),
+                                      _ptr(d_out8), _stream_handle(stream)))

@@ -18,11 +18,13 @@
 #include "fbp_backproject.cuh"
 #include "fbp_filter.cuh"
 #include "fbp_filter2.cuh"
+#include "fbp_metrics.cuh"
 
 namespace {
 
 constexpr double kPi = 3.14159265358979323846264338327950288;
 constexpr int kNumSm = 148;  // B200
+constexpr int kMetricGrid = 4 * kNumSm;
 
 thread_local std::string g_create_error;
 
@@ -68,6 +70,7 @@ struct fbp_plan {
     void* d_u = nullptr;        // [2][tab_len] dtype: UA | UB, U[j] = g[a_tot - 1 - j]
     void* d_rho2 = nullptr;     // [D] dtype: conditioning term of the paired-parity filter
 
+    double* d_mscratch = nullptr;   // fbp_metrics: [kMetricGrid][3] CTA partials, then mid[3]
     bool use_pdl = true;
     // batch pipeline (run_pipelined): filter of slice group g+1 overlaps back-projection of group g
     static constexpr int kMaxGroups = 16;
@@ -680,6 +683,7 @@ fbp_status fbp_create(fbp_plan** out, int n_angles, int n_det, const double* ang
         FBP_TRY(cudaMalloc(&p->d_tickets, sizeof(int) * nt));
         FBP_TRY(cudaMemset(p->d_tickets, 0, sizeof(int) * nt));
     }
+    FBP_TRY(cudaMalloc(&p->d_mscratch, sizeof(double) * (3 * kMetricGrid + 4)));
     for (int i = 0; i < 4; ++i) FBP_TRY(cudaEventCreate(&p->ev[i]));
     p->pipe_min_batch = env_int("FBP_PIPE_MIN_BATCH", 8);
     p->pipe_group = env_int("FBP_PIPE_GROUP", 0);
@@ -703,7 +707,7 @@ void fbp_destroy(fbp_plan* p)
     {
         DeviceGuard guard(p->device);
         cudaFree(p->d_cs2); cudaFree(p->d_taps); cudaFree(p->d_rho); cudaFree(p->d_ent); cudaFree(p->d_part); cudaFree(p->d_tickets);
-        cudaFree(p->d_hsino); cudaFree(p->d_himg); cudaFree(p->d_u); cudaFree(p->d_rho2);
+        cudaFree(p->d_hsino); cudaFree(p->d_himg); cudaFree(p->d_u); cudaFree(p->d_rho2); cudaFree(p->d_mscratch);
         for (int i = 0; i < 4; ++i) if (p->ev[i]) cudaEventDestroy(p->ev[i]);
         if (p->st_f) { cudaStreamSynchronize(p->st_f); cudaStreamDestroy(p->st_f); }
         for (int i = 0; i < 2; ++i) if (p->st_b[i]) { cudaStreamSynchronize(p->st_b[i]); cudaStreamDestroy(p->st_b[i]); }
@@ -776,6 +780,45 @@ fbp_status fbp_reconstruct_host(fbp_plan* p, const void* h_sino, void* h_image, 
     if (st != FBP_OK) return st;
     FBP_CUDA(p, cudaMemcpyAsync(h_image, p->d_himg, img_bytes * batch, cudaMemcpyDeviceToHost, s));
     FBP_CUDA(p, cudaStreamSynchronize(s));
+    return FBP_OK;
+}
+
+}  // extern "C"
+
+template <typename T>
+static cudaError_t launch_metrics(fbp_plan* p, const void* x, const void* y, long long n, double max_val,
+                                  double c1, double c2, double* d_out, cudaStream_t st)
+{
+    double* partial = p->d_mscratch;
+    double* mid = p->d_mscratch + 3 * kMetricGrid;
+    long long want = (n + fbp::kMetricThreads - 1) / fbp::kMetricThreads;
+    const int grid = (int)(want < kMetricGrid ? (want < 1 ? 1 : want) : kMetricGrid);
+    const T* a = static_cast<const T*>(x);
+    const T* b = static_cast<const T*>(y);
+    fbp::metrics_partial_kernel<T, 0><<<grid, fbp::kMetricThreads, 0, st>>>(a, b, n, mid, partial);
+    fbp::metrics_final_kernel<0><<<1, 32, 0, st>>>(partial, grid, n, mid, max_val, c1, c2, d_out);
+    fbp::metrics_partial_kernel<T, 1><<<grid, fbp::kMetricThreads, 0, st>>>(a, b, n, mid, partial);
+    fbp::metrics_final_kernel<1><<<1, 32, 0, st>>>(partial, grid, n, mid, max_val, c1, c2, d_out);
+    return cudaGetLastError();
+}
+
+extern "C" {
+
+fbp_status fbp_metrics(fbp_plan* p, const void* d_x, const void* d_y, long long n, double max_val, double c1,
+                       double c2, double* d_out8, void* stream)
+{
+    if (!p) return FBP_EINVAL;
+    if (!d_x || !d_y || !d_out8) return fail(p, FBP_EINVAL, "NULL device pointer");
+    if (n < 1) return fail(p, FBP_EINVAL, "n must be >= 1");
+    if (!(max_val > 0.0) || !std::isfinite(max_val)) return fail(p, FBP_EINVAL, "max_val must be finite and > 0");
+    if ((reinterpret_cast<uintptr_t>(d_out8) & 7u) != 0) return fail(p, FBP_EINVAL, "d_out8 must be 8-byte aligned");
+    if (c1 < 0.0) c1 = (0.01 * max_val) * (0.01 * max_val);
+    if (c2 < 0.0) c2 = (0.03 * max_val) * (0.03 * max_val);
+    DeviceGuard guard(p->device);
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    cudaError_t e = p->dtype == FBP_F32 ? launch_metrics<float>(p, d_x, d_y, n, max_val, c1, c2, d_out8, s)
+                                        : launch_metrics<double>(p, d_x, d_y, n, max_val, c1, c2, d_out8, s);
+    if (e != cudaSuccess) return cuda_fail(p, e, "metrics launch");
     return FBP_OK;
 }
 
