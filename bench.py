@@ -42,6 +42,9 @@ def parse_args():
     ap.add_argument("--dtype", default="f32", choices=["f32", "f64"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--window", default="ramlak", choices=["ramlak", "shepp-logan", "cosine", "hamming", "hann"],
+                    help="reconstruction filter (SURVEY.md 8(f) row 1); the headline is ramlak")
+    ap.add_argument("--extras", action="store_true", help="also time fbp_metrics (PSNR/SSIM) on the output stack")
     return ap.parse_args()
 
 
@@ -237,6 +240,8 @@ def run_ours(args):
     d_img = torch.empty((B, N, N), dtype=tdt, device="cuda")
     h_img = torch.empty((B, N, N), dtype=tdt).pin_memory()
     plan = fbp.Plan(list(ang), D, N, dtype=args.dtype, max_batch=B)
+    if args.window != "ramlak":
+        plan.set_window(args.window)
     info = plan.info()
     stream = torch.cuda.current_stream()
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")  # > 126 MB L2
@@ -288,6 +293,19 @@ def run_ours(args):
     barrier()
     e2e_s = (time.perf_counter() - t0) / e2e_steps
 
+    extras = None
+    if args.extras:
+        # fbp_metrics on the whole output stack against a copy: 2 passes x 2 arrays read (HBM-bound)
+        other = d_img.clone()
+        out8 = torch.empty(8, dtype=torch.float64, device="cuda")
+        mfn = lambda: fbp.fbp_metrics(plan.handle, d_img, other, d_img.numel(), 1.0, -1.0, -1.0, out8, stream)  # noqa: E731
+        for _ in range(3):
+            mfn()
+        m_ms = timed_loop(mfn, 20) / 20
+        m_bytes = 4.0 * d_img.numel() * d_img.element_size()
+        extras = {"metrics_ms": m_ms, "metrics_gbs": m_bytes / (m_ms * 1e-3) / 1e9, "metrics_bytes": m_bytes,
+                  "metrics_launches": 4, "psnr": float(out8[1].item()), "ssim": float(out8[2].item())}
+
     if world > 1:
         t = torch.tensor([ms_step, e2e_s, b_ms, f_ms], device="cuda", dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -295,7 +313,8 @@ def run_ours(args):
     updates = float(B) * N * N * K
     return dict(world=world, rank=rank, cfg=cfg, info=info, ms_step=ms_step, f_ms=f_ms, b_ms=b_ms, e2e_s=e2e_s,
                 updates=updates, clocks=clk.summary(), esize=h_sino.element_size(),
-                h2d=h_sino.numel() * h_sino.element_size(), d2h=h_img.numel() * h_img.element_size(), plan=plan)
+                h2d=h_sino.numel() * h_sino.element_size(), d2h=h_img.numel() * h_img.element_size(), plan=plan,
+                extras=extras)
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the back-projection kernel, per launch, from
@@ -324,6 +343,8 @@ def main():
     filt_bytes = 2.0 * cfg.batch * cfg.n_angles * cfg.n_det * r["esize"]
     de, dn = (cfg.n_det + 1) // 2, cfg.n_det // 2
     filt_fma = cfg.batch * cfg.n_angles * (2.0 * de * dn + cfg.n_det)
+    if args.window != "ramlak":
+        filt_fma = cfg.batch * cfg.n_angles * float(cfg.n_det) * cfg.n_det      # every tap is non-zero
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": r["ms_step"], "higher_is_better": True,
@@ -351,6 +372,9 @@ def main():
         "gpu_launches": args.steps * r["info"]["kernels_per_reconstruct"],
         "clocks": r["clocks"],
     }
+    line["config"]["window"] = args.window
+    if r["extras"]:
+        line["extras"] = dict(r["extras"], metrics_hbm_frac=r["extras"]["metrics_gbs"] / float(peaks["hbm_gbs"]))
     if world == 1 and not args.no_cpu_baseline:
         frac = oracle_fraction(args.config, 15.0, 3)
         g, cores, sample, _ = time_oracle(args.config, frac, reps=3)

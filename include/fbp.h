@@ -119,6 +119,35 @@ fbp_status fbp_reconstruct_host(fbp_plan *plan, const void *h_sino, void *h_imag
 fbp_status fbp_metrics(fbp_plan *plan, const void *d_x, const void *d_y, long long n, double max_val,
                        double c1, double c2, double *d_out8, void *cuda_stream);
 
+/*
+ * fbp_set_window -- choose the reconstruction filter H of PAPER.md:61 ("Q = P * H"; the paper names
+ * no particular H).  The taps are the inverse DTFT of |f| W(f) on |f| <= 1/2 cycles per sample,
+ *   h_W[m] = 2 * integral_0^{1/2} f W(f) cos(2 pi f m) df   (closed forms, computed in fp64 on the host):
+ *   FBP_WINDOW_RAMLAK       W = 1  (default; the only window with zero even taps)
+ *   FBP_WINDOW_SHEPP_LOGAN  W = sin(pi f)/(pi f)      h[m] = -2 / (pi^2 (4 m^2 - 1))
+ *   FBP_WINDOW_COSINE       W = cos(pi f)
+ *   FBP_WINDOW_HAMMING      W = 0.54 + 0.46 cos(2 pi f)
+ *   FBP_WINDOW_HANN         W = 0.5 + 0.5 cos(2 pi f)
+ * Applies to fbp_filter and fbp_reconstruct from the next call on.  Synchronous: waits for the device,
+ * rebuilds and uploads the tap tables.  FBP_EUNSUPPORTED if the row is too long for the dense kernel.
+ */
+typedef enum {
+    FBP_WINDOW_RAMLAK = 0,
+    FBP_WINDOW_SHEPP_LOGAN = 1,
+    FBP_WINDOW_COSINE = 2,
+    FBP_WINDOW_HAMMING = 3,
+    FBP_WINDOW_HANN = 4
+} fbp_window;
+fbp_status fbp_set_window(fbp_plan *plan, fbp_window window);
+
+/*
+ * fbp_set_angle_weights -- per-angle weights for non-uniform angle sets: f = sum_i w_i q_i instead of
+ * (pi/K) sum_i q_i (eq. 2, which carries no weight at all).
+ * h_weights: HOST pointer to K finite values, copied; NULL restores pi/K for every angle.  Applies to
+ * fbp_backproject and fbp_reconstruct from the next call on.  Synchronous.
+ */
+fbp_status fbp_set_angle_weights(fbp_plan *plan, const double *h_weights);
+
 /* fbp_destroy -- free the plan, its tables and scratch.  NULL-safe.  Synchronous. */
 void fbp_destroy(fbp_plan *plan);
 

@@ -10,7 +10,7 @@ from .binding import (  # noqa: F401
     EXPORTS, FBP_F32, FBP_F64, FBP_OK, FBP_EINVAL, FBP_ENOMEM, FBP_ECUDA, FBP_EUNSUPPORTED,
     FbpError, load_library,
     fbp_create, fbp_filter, fbp_backproject, fbp_reconstruct, fbp_reconstruct_host,
-    fbp_destroy, fbp_last_error, fbp_plan_info, fbp_set_profiling, fbp_get_kernel_ms, fbp_metrics,
+    fbp_destroy, fbp_last_error, fbp_plan_info, fbp_set_profiling, fbp_get_kernel_ms, fbp_metrics, fbp_set_window, fbp_set_angle_weights, WINDOWS,
 )
 from .build import build  # noqa: F401
 
@@ -73,6 +73,14 @@ class Plan:
         out = self._empty(sino, (self.image_n, self.image_n)) if out is None else out
         fbp_reconstruct(self.handle, sino, out, b, stream)
         return out
+
+    def set_window(self, window):
+        fbp_set_window(self.handle, window)
+
+    def set_angle_weights(self, weights):
+        if weights is not None and len(weights) != self.n_angles:
+            raise ValueError("expected one weight per angle")
+        fbp_set_angle_weights(self.handle, weights)
 
     def metrics(self, x, y, max_val, c1=-1.0, c2=-1.0, stream=None) -> dict:
         """PSNR / SSIM (eq. 3, 4 of the paper) of two CUDA tensors of the plan dtype; one device-to-host read."""

@@ -18,7 +18,7 @@ STATUS_NAMES = {0: "FBP_OK", 1: "FBP_EINVAL", 2: "FBP_ENOMEM", 3: "FBP_ECUDA", 4
 EXPORTS = (
     "fbp_create", "fbp_filter", "fbp_backproject", "fbp_reconstruct", "fbp_reconstruct_host",
     "fbp_destroy", "fbp_last_error", "fbp_plan_info", "fbp_set_profiling", "fbp_get_kernel_ms",
-    "fbp_metrics",
+    "fbp_metrics", "fbp_set_window", "fbp_set_angle_weights",
 )
 
 PLAN_INFO_FIELDS = (
@@ -57,6 +57,10 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         fn.restype = ci
     lib.fbp_metrics.argtypes = [vp, vp, vp, ctypes.c_longlong, cd, cd, cd, vp, vp]
     lib.fbp_metrics.restype = ci
+    lib.fbp_set_window.argtypes = [vp, ci]
+    lib.fbp_set_window.restype = ci
+    lib.fbp_set_angle_weights.argtypes = [vp, ctypes.POINTER(cd)]
+    lib.fbp_set_angle_weights.restype = ci
     lib.fbp_destroy.argtypes = [vp]
     lib.fbp_destroy.restype = None
     lib.fbp_last_error.argtypes = [vp]
@@ -168,3 +172,21 @@ def fbp_metrics(plan, d_x, d_y, n, max_val, c1, c2, d_out8, stream=None):
     lib = load_library()
     _check(lib, plan, lib.fbp_metrics(plan, _ptr(d_x), _ptr(d_y), int(n), float(max_val), float(c1), float(c2),
                                       _ptr(d_out8), _stream_handle(stream)))
+
+
+WINDOWS = {"ramlak": 0, "shepp-logan": 1, "cosine": 2, "hamming": 3, "hann": 4}
+
+
+def fbp_set_window(plan, window):
+    lib = load_library()
+    _check(lib, plan, lib.fbp_set_window(plan, int(WINDOWS.get(window, window))))
+
+
+def fbp_set_angle_weights(plan, weights):
+    lib = load_library()
+    if weights is None:
+        arr = None
+    else:
+        vals = [float(w) for w in weights]
+        arr = (ctypes.c_double * max(len(vals), 1))(*vals)
+    _check(lib, plan, lib.fbp_set_angle_weights(plan, arr))

@@ -24,7 +24,7 @@ namespace {
 
 constexpr double kPi = 3.14159265358979323846264338327950288;
 constexpr int kNumSm = 148;  // B200
-constexpr int kMetricGrid = 4 * kNumSm;
+constexpr int kMetricGrid = 8 * kNumSm;
 
 thread_local std::string g_create_error;
 
@@ -69,6 +69,13 @@ struct fbp_plan {
     fbp::Filter2Params f2{};
     void* d_u = nullptr;        // [2][tab_len] dtype: UA | UB, U[j] = g[a_tot - 1 - j]
     void* d_rho2 = nullptr;     // [D] dtype: conditioning term of the paired-parity filter
+    // apodised windows (fbp_set_window): the dense form of the same kernel; window 0 = Ram-Lak
+    int window = 0;
+    int f2d_r = 7, f2d_threads = 0, f2d_smem = 0, f2d_grid_cap = 0;
+    fbp::Filter2Params f2d{};
+    void* d_ud = nullptr;       // [2][tab_len] dtype: UA | UB of the dense table, U[j] = H[2 a_tot - j]
+    void* d_rhod = nullptr;     // [D] dtype
+    void* d_wrow = nullptr;     // [K] dtype: angle weight / (pi/K) (fbp_set_angle_weights); NULL = uniform
 
     double* d_mscratch = nullptr;   // fbp_metrics: [kMetricGrid][3] CTA partials, then mid[3]
     bool use_pdl = true;
@@ -211,6 +218,66 @@ void configure_filter2(fbp_plan* p)
     const size_t elems = 2 * (size_t)f.tab_len + 4 * (size_t)f.b_pad + (size_t)f.n_ob * 32 +
                          (size_t)sb * 2 * f.a_tot + (size_t)(f.ent_pitch + 2) + (size_t)D;
     p->f2_smem = (int)(elems * p->esize + 16);
+}
+
+// Dense form (apodised windows): R odd, chunks of 2R inputs, same warp layout.
+void configure_filter2_dense(fbp_plan* p)
+{
+    const int D = p->D;
+    const int na = (D + 1) / 2;
+    static const int cand[] = {5, 7, 9};
+    int best_r = 5;
+    double best = -1.0;
+    for (int R : cand) {
+        const int n_ob = (na + 32 * R - 1) / (32 * R);
+        if (n_ob > 16) continue;
+        if (p->dtype == FBP_F64 && R > 5) continue;    // 6R fp64 registers of accumulators and taps
+        const double util = (double)na / ((double)n_ob * 32 * R);
+        const double score = util * (2.0 * R) / (2.0 * R + 2.0);
+        if (score > best) { best = score; best_r = R; }
+    }
+    const int R = best_r;
+    p->f2d_r = R;
+    fbp::Filter2Params& f = p->f2d;
+    f.n_det = D;
+    f.n_ob = (na + 32 * R - 1) / (32 * R);
+    f.a_tot = f.n_ob * 32 * R;
+    f.n_chunks = (D + 2 * R - 1) / (2 * R);
+    f.b_pad = f.n_chunks * R;
+    const double rows_per_sm = (double)p->max_batch * p->K / kNumSm;
+    const int target = rows_per_sm >= 64.0 ? 4 : (f.n_ob >= 4 ? 16 : 8);
+    int sb = (target + f.n_ob / 2) / f.n_ob;
+    if (sb < 1) sb = 1;
+    if (sb > 8) sb = 8;
+    if (sb > f.n_chunks) sb = f.n_chunks;
+    while (sb > 1 && f.n_ob * sb > 16) --sb;
+    f.n_sb = sb;
+    f.tab_len = round_up(2 * f.a_tot + 2 * f.b_pad + 4, 4);
+    f.ent_pitch = p->bp.ent_pitch; f.ent_guard = p->bp.ent_guard;
+    p->f2d_threads = f.n_ob * sb * 32;
+    const size_t elems = 2 * (size_t)f.tab_len + 4 * (size_t)f.b_pad + (size_t)f.n_ob * 32 +
+                         (size_t)sb * 2 * f.a_tot + (size_t)(f.ent_pitch + 2) + (size_t)D;
+    p->f2d_smem = (int)(elems * p->esize + 16);
+}
+
+// One tap of the apodised ramp |f| W(f), |f| <= 1/2: h_W[m] = 2 int_0^{1/2} f W(f) cos(2 pi f m) df in closed
+// form (include/fbp.h, fbp_set_window; derivations in DESIGN.md "Windows").  Any integer m.
+double window_tap(int window, long long m)
+{
+    auto ramlak = [](long long q) -> double {
+        if (q == 0) return 0.25;
+        if (q % 2 == 0) return 0.0;
+        return -1.0 / (kPi * kPi * (double)q * (double)q);
+    };
+    auto half_moment = [](double a) { return std::sin(0.5 * a) / (2.0 * a) + (std::cos(0.5 * a) - 1.0) / (a * a); };
+    const double md = (double)m;
+    switch (window) {
+        case FBP_WINDOW_SHEPP_LOGAN: return -2.0 / (kPi * kPi * (4.0 * md * md - 1.0));
+        case FBP_WINDOW_COSINE: return half_moment(kPi * (2.0 * md + 1.0)) + half_moment(kPi * (2.0 * md - 1.0));
+        case FBP_WINDOW_HAMMING: return 0.54 * ramlak(m) + 0.23 * (ramlak(m + 1) + ramlak(m - 1));
+        case FBP_WINDOW_HANN: return 0.5 * ramlak(m) + 0.25 * (ramlak(m + 1) + ramlak(m - 1));
+        default: return ramlak(m);
+    }
 }
 
 // ---- back-projection launch configuration ------------------------------------------
@@ -362,35 +429,45 @@ cudaError_t launch_filter(const fbp_plan* p, const void* sino, void* filt, void*
     }
 }
 
-template <typename T, int R>
+template <typename T, int R, bool DENSE>
 cudaError_t launch_filter2_r(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st)
 {
-    fbp::Filter2Params f = p->f2;
+    fbp::Filter2Params f = DENSE ? p->f2d : p->f2;
     f.n_rows = batch * p->K;
-    auto kern = fbp::filter2_kernel<T, R>;
-    if (p->f2_grid_cap == 0) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, p->f2_smem);
+    const int threads = DENSE ? p->f2d_threads : p->f2_threads, smem = DENSE ? p->f2d_smem : p->f2_smem;
+    int& cap = DENSE ? p->f2d_grid_cap : p->f2_grid_cap;
+    auto kern = fbp::filter2_kernel<T, R, DENSE>;
+    if (cap == 0) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         int per_sm = 0;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, p->f2_threads, p->f2_smem);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem);
         if (e != cudaSuccess) return e;
         if (per_sm < 1) return cudaErrorLaunchOutOfResources;
-        p->f2_grid_cap = per_sm * kNumSm;
+        cap = per_sm * kNumSm;
     }
-    const int grid = f.n_rows < p->f2_grid_cap ? f.n_rows : p->f2_grid_cap;
-    kern<<<grid, p->f2_threads, p->f2_smem, st>>>(static_cast<const T*>(sino), static_cast<T*>(filt),
-                                                  static_cast<uint4*>(ent), static_cast<const T*>(p->d_u),
-                                                  static_cast<const T*>(p->d_rho2), f, (T)(1.0 / p->d));
+    const int grid = f.n_rows < cap ? f.n_rows : cap;
+    kern<<<grid, threads, smem, st>>>(static_cast<const T*>(sino), static_cast<T*>(filt), static_cast<uint4*>(ent),
+                                      static_cast<const T*>(DENSE ? p->d_ud : p->d_u),
+                                      static_cast<const T*>(DENSE ? p->d_rhod : p->d_rho2),
+                                      static_cast<const T*>(p->d_wrow), p->K, f, (T)(1.0 / p->d));
     return cudaGetLastError();
 }
 
 template <typename T>
 cudaError_t launch_filter2(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st)
 {
+    if (p->window != 0) {
+        switch (p->f2d_r) {
+            case 5: return launch_filter2_r<T, 5, true>(p, sino, filt, ent, batch, st);
+            case 7: return launch_filter2_r<T, 7, true>(p, sino, filt, ent, batch, st);
+            default: return launch_filter2_r<T, 9, true>(p, sino, filt, ent, batch, st);
+        }
+    }
     switch (p->f2_r) {
-        case 6: return launch_filter2_r<T, 6>(p, sino, filt, ent, batch, st);
-        case 10: return launch_filter2_r<T, 10>(p, sino, filt, ent, batch, st);
-        default: return launch_filter2_r<T, 14>(p, sino, filt, ent, batch, st);
+        case 6: return launch_filter2_r<T, 6, false>(p, sino, filt, ent, batch, st);
+        case 10: return launch_filter2_r<T, 10, false>(p, sino, filt, ent, batch, st);
+        default: return launch_filter2_r<T, 14, false>(p, sino, filt, ent, batch, st);
     }
 }
 
@@ -402,7 +479,7 @@ cudaError_t launch_entries(const fbp_plan* p, const void* filt, int batch, cudaS
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kern<<<batch * p->K, 256, smem, st>>>(static_cast<const T*>(filt), static_cast<uint4*>(p->d_ent), p->D,
-                                          p->bp.ent_pitch, p->bp.ent_guard);
+                                          p->bp.ent_pitch, p->bp.ent_guard, static_cast<const T*>(p->d_wrow), p->K);
     return cudaGetLastError();
 }
 
@@ -593,6 +670,7 @@ fbp_status fbp_create(fbp_plan** out, int n_angles, int n_det, const double* ang
     configure_bp(p, cs);
     configure_filter(p);   // after configure_bp: needs the entry pitch
     configure_filter2(p);
+    configure_filter2_dense(p);
     p->filter_v = env_int("FBP_FILTER_V", 2) == 1 ? 1 : 2;
     p->use_pdl = env_int("FBP_PDL", 1) != 0;
 
@@ -708,6 +786,7 @@ void fbp_destroy(fbp_plan* p)
         DeviceGuard guard(p->device);
         cudaFree(p->d_cs2); cudaFree(p->d_taps); cudaFree(p->d_rho); cudaFree(p->d_ent); cudaFree(p->d_part); cudaFree(p->d_tickets);
         cudaFree(p->d_hsino); cudaFree(p->d_himg); cudaFree(p->d_u); cudaFree(p->d_rho2); cudaFree(p->d_mscratch);
+        cudaFree(p->d_ud); cudaFree(p->d_rhod); cudaFree(p->d_wrow);
         for (int i = 0; i < 4; ++i) if (p->ev[i]) cudaEventDestroy(p->ev[i]);
         if (p->st_f) { cudaStreamSynchronize(p->st_f); cudaStreamDestroy(p->st_f); }
         for (int i = 0; i < 2; ++i) if (p->st_b[i]) { cudaStreamSynchronize(p->st_b[i]); cudaStreamDestroy(p->st_b[i]); }
@@ -819,6 +898,71 @@ fbp_status fbp_metrics(fbp_plan* p, const void* d_x, const void* d_y, long long 
     cudaError_t e = p->dtype == FBP_F32 ? launch_metrics<float>(p, d_x, d_y, n, max_val, c1, c2, d_out8, s)
                                         : launch_metrics<double>(p, d_x, d_y, n, max_val, c1, c2, d_out8, s);
     if (e != cudaSuccess) return cuda_fail(p, e, "metrics launch");
+    return FBP_OK;
+}
+
+fbp_status fbp_set_window(fbp_plan* p, fbp_window window)
+{
+    if (!p) return FBP_EINVAL;
+    if ((int)window < 0 || (int)window > (int)FBP_WINDOW_HANN) return fail(p, FBP_EINVAL, "unknown window");
+    if (window == FBP_WINDOW_RAMLAK) { p->window = 0; return FBP_OK; }
+    if (p->filter_v != 2 || p->f2d_threads > 512 || p->f2d_smem > 220 * 1024)
+        return fail(p, FBP_EUNSUPPORTED, "n_det too large for the dense (windowed) row filter");
+    DeviceGuard guard(p->device);
+    FBP_CUDA(p, cudaDeviceSynchronize());          // nothing of this plan may be in flight while its tables change
+    const fbp::Filter2Params& f = p->f2d;
+    const int tl = f.tab_len, D = p->D, x_len = 2 * f.b_pad;
+    std::vector<double> u64(2 * (size_t)tl), rho64(D);
+    for (int j = 0; j < tl; ++j) {
+        u64[j] = window_tap((int)window, 2LL * f.a_tot - j);
+        u64[tl + j] = window_tap((int)window, 2LL * f.a_tot - j - 1);
+    }
+    // conditioning term: the dense filter's response to a constant row over the padded inputs,
+    // rho[n] = sum_{k < x_len} H[n - k], summed smallest magnitudes first
+    for (int n = 0; n < D; ++n) {
+        std::vector<double> terms(x_len);
+        for (int k = 0; k < x_len; ++k) terms[k] = window_tap((int)window, (long long)n - k);
+        std::sort(terms.begin(), terms.end(), [](double a, double b) { return std::fabs(a) < std::fabs(b); });
+        double ssum = 0.0;
+        for (double t : terms) ssum += t;
+        rho64[n] = ssum;
+    }
+    std::vector<float> u32, rho32;
+    const void* usrc = u64.data();
+    const void* rsrc = rho64.data();
+    if (p->dtype == FBP_F32) {
+        u32.assign(u64.begin(), u64.end()); usrc = u32.data();
+        rho32.assign(rho64.begin(), rho64.end()); rsrc = rho32.data();
+    }
+    if (!p->d_ud) FBP_CUDA(p, cudaMalloc(&p->d_ud, p->esize * 2 * (size_t)tl));
+    if (!p->d_rhod) FBP_CUDA(p, cudaMalloc(&p->d_rhod, p->esize * (size_t)D));
+    FBP_CUDA(p, cudaMemcpy(p->d_ud, usrc, p->esize * 2 * (size_t)tl, cudaMemcpyHostToDevice));
+    FBP_CUDA(p, cudaMemcpy(p->d_rhod, rsrc, p->esize * (size_t)D, cudaMemcpyHostToDevice));
+    p->window = (int)window;
+    return FBP_OK;
+}
+
+fbp_status fbp_set_angle_weights(fbp_plan* p, const double* h_weights)
+{
+    if (!p) return FBP_EINVAL;
+    DeviceGuard guard(p->device);
+    FBP_CUDA(p, cudaDeviceSynchronize());
+    if (!h_weights) {
+        cudaFree(p->d_wrow);
+        p->d_wrow = nullptr;
+        return FBP_OK;
+    }
+    if (p->filter_v != 2) return fail(p, FBP_EUNSUPPORTED, "angle weights need the paired-parity filter");
+    for (int i = 0; i < p->K; ++i)
+        if (!std::isfinite(h_weights[i])) return fail(p, FBP_EINVAL, "non-finite angle weight");
+    // the back-projector keeps its pi/K factor: the entries of row i carry w_i / (pi/K)
+    std::vector<double> m64(p->K);
+    for (int i = 0; i < p->K; ++i) m64[i] = h_weights[i] * (double)p->K / kPi;
+    std::vector<float> m32;
+    const void* src = m64.data();
+    if (p->dtype == FBP_F32) { m32.assign(m64.begin(), m64.end()); src = m32.data(); }
+    if (!p->d_wrow) FBP_CUDA(p, cudaMalloc(&p->d_wrow, p->esize * (size_t)p->K));
+    FBP_CUDA(p, cudaMemcpy(p->d_wrow, src, p->esize * (size_t)p->K, cudaMemcpyHostToDevice));
     return FBP_OK;
 }
 

@@ -67,11 +67,16 @@ __device__ __forceinline__ void store_entry(uint4* erow, int pitch, int i, doubl
 }
 
 template <typename T>
-__device__ __forceinline__ void store_entries(const T* yz, uint4* erow, int pitch, int tid, int nthr)
+__device__ __forceinline__ void store_entries(const T* yz, uint4* erow, int pitch, int tid, int nthr,
+                                              const T* wmul = nullptr)
 {
+    // wmul: this row's angle weight divided by pi/K (fbp_set_angle_weights); NULL = the uniform pi/K
+    const bool scaled = wmul != nullptr;
+    const T m = scaled ? *wmul : T(1);
     for (int i = tid; i < pitch; i += nthr) {
-        const T a0 = yz[i + 1], a1 = yz[i + 2];
-        const T b0 = yz[pitch - 1 - i], b1 = yz[pitch - i];
+        T a0 = yz[i + 1], a1 = yz[i + 2];
+        T b0 = yz[pitch - 1 - i], b1 = yz[pitch - i];
+        if (scaled) { a0 *= m; a1 *= m; b0 *= m; b1 *= m; }
         store_entry(erow, pitch, i, T(0.5) * (a0 + a1), T(0.5) * (b0 + b1), a1 - a0, b0 - b1);
     }
 }
@@ -187,7 +192,8 @@ filter_kernel(const T* __restrict__ P, T* __restrict__ Q, uint4* __restrict__ E,
 // as the filter epilogue, so fbp_reconstruct == fbp_backproject(fbp_filter) bit for bit.
 template <typename T>
 __global__ void __launch_bounds__(256)
-entries_kernel(const T* __restrict__ Q, uint4* __restrict__ E, int n_det, int ent_pitch, int ent_guard)
+entries_kernel(const T* __restrict__ Q, uint4* __restrict__ E, int n_det, int ent_pitch, int ent_guard,
+               const T* __restrict__ wrow, int n_angles)
 {
     extern __shared__ __align__(16) unsigned char ent_smem_raw[];
     T* yz = reinterpret_cast<T*>(ent_smem_raw);
@@ -199,7 +205,8 @@ entries_kernel(const T* __restrict__ Q, uint4* __restrict__ E, int n_det, int en
         yz[k] = (n >= 0 && n < n_det) ? q[n] : T(0);
     }
     __syncthreads();
-    store_entries<T>(yz, E + (size_t)row * EntryPlanes<T>::value * ent_pitch, ent_pitch, threadIdx.x, blockDim.x);
+    store_entries<T>(yz, E + (size_t)row * EntryPlanes<T>::value * ent_pitch, ent_pitch, threadIdx.x, blockDim.x,
+                     wrow ? wrow + row % n_angles : nullptr);
 }
 
 }  // namespace fbp

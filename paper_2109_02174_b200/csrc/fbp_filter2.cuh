@@ -93,12 +93,20 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;"
 
 // U_gmem: [2][tab_len] = UA | UB (see above), U[j] = g[a_tot - 1 - j].  rho: [D].
 // Block = n_ob * n_sb warps.  Grid <= number of co-resident CTAs (persistent).
-template <typename T, int R>
+//
+// DENSE = true is the general form for apodised windows (every tap non-zero; SURVEY.md 8(f) row 1,
+// the paper's H is generic): input k (splat) meets the tap pair (H[2a+1-k], H[2a-k])
+// of output pair a, U[j] = H[2 a_tot - j], pair index j = 2 a_tot - 1 - 2a + k.  The pairs of even and
+// of odd k form two register windows that each slide by one slot every second step; lane stride
+// is 2R words, so R is odd.  Twice the multiply-adds of the Ram-Lak form (twice the taps).
+// wrow: per-row multipliers of the entries (fbp_set_angle_weights), NULL = none.
+template <typename T, int R, bool DENSE>
 __global__ void __launch_bounds__(512)
 filter2_kernel(const T* __restrict__ P, T* __restrict__ Q, uint4* __restrict__ E,
-               const T* __restrict__ U_gmem, const T* __restrict__ rho, Filter2Params prm, T inv_d)
+               const T* __restrict__ U_gmem, const T* __restrict__ rho, const T* __restrict__ wrow,
+               int n_angles, Filter2Params prm, T inv_d)
 {
-    static_assert(R % 4 == 2, "R = 2 mod 4 keeps the tap-pair loads conflict-free");
+    static_assert(DENSE ? (R % 2 == 1) : (R % 4 == 2), "lane stride (R or 2R words) must be 2 mod 4: conflict-free pair loads");
     using P2 = Pair2<T>;
     extern __shared__ __align__(16) unsigned char f2_smem_raw[];
     // layout: UA[tab_len] UB[tab_len] X[2][2*b_pad] C[n_ob*32] part[n_sb][2*a_tot] yz[ent_pitch+2] rho[D]
@@ -133,7 +141,8 @@ filter2_kernel(const T* __restrict__ P, T* __restrict__ Q, uint4* __restrict__ E
 
     // per-thread constants
     const int a0 = (ob * 32 + lane) * R;                 // first output pair of this thread
-    const int cl = prm.a_tot - 1 - a0;                   // odd: U index of (a0, b = 0)
+    const int cl = (DENSE ? 2 * prm.a_tot - 1 - 2 * a0    // odd: U index of (a0, k = 0)
+                          : prm.a_tot - 1 - a0);          // odd: U index of (a0, b = 0)
     const T* ua = UA + cl;                               // pair at even U index j: ua[j - cl]
     const T* ub = UB + cl - 1;                           // pair at odd  U index j: ub[j - cl]
     const int a_max = (D - 1) >> 1;
@@ -155,30 +164,58 @@ filter2_kernel(const T* __restrict__ P, T* __restrict__ Q, uint4* __restrict__ E
         cp_async_wait<1>();    // everything but the prefetch just issued has landed
         __syncthreads();
 
-        // ---- compute: R output pairs x this warp's slice of the input pairs ----
+        // ---- compute: R output pairs x this warp's slice of the inputs (chunks of 2R inputs) ----
         {
             const T c = X[2 * ac];
             if (sb == 0) Cs[ob * 32 + lane] = c;
             const P2 nc = P2::splat(-c);
-            P2 acc[R], W[R];
-            const int b_begin = ch_begin * R;
+            P2 acc[R];
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-                acc[r] = P2::zero();
-                // U index cl - r + b_begin: even for odd r (UA), odd for even r (UB)
-                W[r] = (r & 1) ? P2::load(ua + (b_begin - r)) : P2::load(ub + (b_begin - r));
-            }
-            for (int ch = ch_begin; ch < ch_end; ++ch) {
-                const int b0 = ch * R;
+            for (int r = 0; r < R; ++r) acc[r] = P2::zero();
+            if (!DENSE) {
+                P2 W[R];
+                const int b_begin = ch_begin * R;
 #pragma unroll
-                for (int s = 0; s < R; ++s) {
-                    // the pair of (r = 0, b = b0 + s): U index cl + b0 + s, even iff s odd
-                    if (s > 0) W[R - s] = (s & 1) ? P2::load(ua + (b0 + s)) : P2::load(ub + (b0 + s));
-                    const P2 x = P2::load(X + 2 * (b0 + s)).plus(nc);
+                for (int r = 0; r < R; ++r)   // U index cl - r + b_begin: even for odd r (UA), odd for even r (UB)
+                    W[r] = (r & 1) ? P2::load(ua + (b_begin - r)) : P2::load(ub + (b_begin - r));
+                for (int ch = ch_begin; ch < ch_end; ++ch) {
+                    const int b0 = ch * R;
 #pragma unroll
-                    for (int r = 0; r < R; ++r) acc[r].fma(W[(r - s + R) % R], x);
+                    for (int s = 0; s < R; ++s) {
+                        // the pair of (r = 0, b = b0 + s): U index cl + b0 + s, even iff s odd
+                        if (s > 0) W[R - s] = (s & 1) ? P2::load(ua + (b0 + s)) : P2::load(ub + (b0 + s));
+                        const P2 x = P2::load(X + 2 * (b0 + s)).plus(nc);
+#pragma unroll
+                        for (int r = 0; r < R; ++r) acc[r].fma(W[(r - s + R) % R], x);
+                    }
+                    W[0] = P2::load(ub + (b0 + R));
                 }
-                W[0] = P2::load(ub + (b0 + R));
+            } else {
+                P2 WE[R], WO[R];
+                const int k_begin = ch_begin * 2 * R;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {     // U index cl - 2r + k: odd for even k (UB), even for odd k (UA)
+                    WE[r] = P2::load(ub + (k_begin - 2 * r));
+                    WO[r] = P2::load(ua + (k_begin + 1 - 2 * r));
+                }
+                for (int ch = ch_begin; ch < ch_end; ++ch) {
+                    const int k0 = ch * 2 * R;
+#pragma unroll
+                    for (int s = 0; s < R; ++s) {
+                        if (s > 0) {
+                            WE[R - s] = P2::load(ub + (k0 + 2 * s));
+                            WO[R - s] = P2::load(ua + (k0 + 2 * s + 1));
+                        }
+                        const P2 x = P2::load(X + (k0 + 2 * s)).plus(nc);
+                        const P2 xe = P2::splat(x.lo()), xo = P2::splat(x.hi());
+#pragma unroll
+                        for (int r = 0; r < R; ++r) acc[r].fma(WE[(r - s + R) % R], xe);
+#pragma unroll
+                        for (int r = 0; r < R; ++r) acc[r].fma(WO[(r - s + R) % R], xo);
+                    }
+                    WE[0] = P2::load(ub + (k0 + 2 * R));
+                    WO[0] = P2::load(ua + (k0 + 2 * R + 1));
+                }
             }
             // natural order: n = 2(a0+r) is the even output (hi), n+1 the odd output (lo)
             T* pp = part + (size_t)sb * y_len + 2 * a0;
@@ -196,7 +233,8 @@ filter2_kernel(const T* __restrict__ P, T* __restrict__ Q, uint4* __restrict__ E
                 T s = part[n];
                 for (int q = 1; q < prm.n_sb; ++q) s += part[(size_t)q * y_len + n];
                 const T c = Cs[(n >> 1) / R];
-                y = (s + T(0.25) * (X[n] - c) + c * rho_s[n]) * inv_d;
+                y = DENSE ? (s + c * rho_s[n]) * inv_d                      // the centre tap is in the sum
+                          : (s + T(0.25) * (X[n] - c) + c * rho_s[n]) * inv_d;
             }
             yz[k] = y;
         }
@@ -208,7 +246,8 @@ filter2_kernel(const T* __restrict__ P, T* __restrict__ Q, uint4* __restrict__ E
             const T* yn = yz + 1 + prm.ent_guard;
             for (int n = tid; n < D; n += nthr) q[n] = yn[n];
         }
-        if (E) store_entries<T>(yz, E + (size_t)row * EntryPlanes<T>::value * prm.ent_pitch, prm.ent_pitch, tid, nthr);
+        if (E) store_entries<T>(yz, E + (size_t)row * EntryPlanes<T>::value * prm.ent_pitch, prm.ent_pitch, tid, nthr,
+                                wrow ? wrow + row % n_angles : nullptr);
     }
     cp_async_wait<0>();
 }

@@ -78,3 +78,124 @@ def test_metrics_error_paths(fbp):
             fbp.fbp_metrics(plan.handle, x, x, 16, 1.0, -1.0, -1.0, 0)
         torch.cuda.synchronize()
         assert bool((out == 7.0).all())
+
+
+# ---- apodised windows (fbp_set_window) and per-angle weights (fbp_set_angle_weights) ----------
+F64_TOL, F32_MAXABS, F32_RMSE = 1e-12, 1e-4, 1e-5
+
+
+def _check_image(gpu, ref, dt, what):
+    err = np.abs(np.asarray(gpu, dtype=np.float64) - ref)
+    if dt == "f64":
+        assert err.max() / np.abs(ref).max() <= F64_TOL, what
+    else:
+        dr = ref.max() - ref.min()
+        assert err.max() / dr <= F32_MAXABS and math.sqrt(float(np.mean(err * err))) / dr <= F32_RMSE, what
+
+
+def _check_filter(gpu, ref, dt, p_max, d, window, what):
+    err = np.abs(np.asarray(gpu, dtype=np.float64) - ref).max()
+    if dt == "f64":
+        assert err / np.abs(ref).max() <= F64_TOL, what
+    else:
+        # n-term recursive fp32 sum, sum |h_W| <= 1/2 + 1/4 for every window here
+        n_det = ref.shape[-1]
+        assert err <= math.sqrt(n_det + 1) * 2.0 ** -24 * 0.75 * p_max / d, (what, err)
+
+
+WINDOW_CASES = [  # (N, K, D, d, batch)
+    (64, 90, 91, 1.0, 1),          # config 1 geometry
+    (33, 7, 48, 0.5, 2),           # D even, N odd
+    (130, 31, 185, 1.0, 1),
+    (256, 24, 363, 1.0, 1),        # config 2 row length
+    (40, 12, 725, 2.0, 1),         # config 3 row length
+]
+
+
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+@pytest.mark.parametrize("window", ["shepp-logan", "cosine", "hamming", "hann"])
+@pytest.mark.parametrize("case", WINDOW_CASES)
+def test_windowed_filter_and_reconstruction_match_oracle(fbp, oracle, case, window, dt):
+    import torch
+    n, k, dd, d, b = case
+    ang = I.uniform_angles(k)
+    sino = I.random_sinogram(21 + dd, b, k, dd).astype(_np_dtype(dt))
+    ref_q = oracle.filter_sinogram_window(sino.astype(np.float64), window, d)
+    ref_f = oracle.backproject(ref_q, ang, n, d)
+    with fbp.Plan(list(ang), dd, n, det_spacing=d, dtype=dt, max_batch=b) as plan:
+        plan.set_window(window)
+        ds = _dev(sino, dt)
+        q = plan.filter(ds)
+        f = plan.reconstruct(ds)
+        f2 = plan.backproject(q)
+        torch.cuda.synchronize()
+        assert torch.equal(f, f2)                                 # reconstruct == backproject(filter)
+        _check_filter(q.cpu().numpy(), ref_q, dt, np.abs(sino).max(), d, window, (case, window))
+        _check_image(f.cpu().numpy(), ref_f, dt, (case, window))
+        plan.set_window("ramlak")                                  # and back: the default path again
+        f0 = plan.reconstruct(ds).cpu().numpy()
+    _check_image(f0, oracle.reconstruct(sino.astype(np.float64), ang, n, d), dt, (case, "ramlak again"))
+
+
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+def test_windowed_cfg3_full_image(fbp, oracle, dt):
+    cfg = I.CONFIGS[3]
+    ang = I.config_angles(3)
+    sino = I.config_sinogram(3).astype(_np_dtype(dt))
+    ref = oracle.backproject(oracle.filter_sinogram_window(sino.astype(np.float64), "hann"), ang, cfg.image_n)
+    with fbp.Plan(list(ang), cfg.n_det, cfg.image_n, dtype=dt) as plan:
+        plan.set_window("hann")
+        a = plan.reconstruct(_dev(sino, dt))
+        b = plan.reconstruct(_dev(sino, dt))
+        assert bool((a == b).all())
+    _check_image(a.cpu().numpy(), ref, dt, "cfg3 hann")
+
+
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+def test_angle_weights_match_oracle(fbp, oracle, dt):
+    """Non-uniform angles with trapezoid weights; NULL restores pi/K."""
+    n, k, dd, b = 70, 41, 101, 2
+    rng = np.random.default_rng(17)
+    ang = np.sort(rng.uniform(0.0, math.pi, k))
+    edges = np.concatenate([[ang[-1] - math.pi], ang, [ang[0] + math.pi]])
+    w = 0.5 * (edges[2:] - edges[:-2])                              # half the gap to each neighbour, periodic in pi
+    assert w.sum() == pytest.approx(math.pi)
+    q = I.random_sinogram(3, b, k, dd).astype(_np_dtype(dt))
+    sino = I.random_sinogram(4, b, k, dd).astype(_np_dtype(dt))
+    with fbp.Plan(list(ang), dd, n, dtype=dt, max_batch=b) as plan:
+        plan.set_angle_weights(list(w))
+        f_bp = plan.backproject(_dev(q, dt)).cpu().numpy()
+        f_rc = plan.reconstruct(_dev(sino, dt)).cpu().numpy()
+        plan.set_angle_weights(None)
+        f_uni = plan.backproject(_dev(q, dt)).cpu().numpy()
+    _check_image(f_bp, oracle.backproject_weighted(q.astype(np.float64), ang, w, n), dt, "weighted bp")
+    ref_q = oracle.filter_sinogram(sino.astype(np.float64))
+    _check_image(f_rc, oracle.backproject_weighted(ref_q, ang, w, n), dt, "weighted reconstruct")
+    _check_image(f_uni, oracle.backproject(q.astype(np.float64), ang, n), dt, "uniform again")
+
+
+def test_window_and_weight_error_paths(fbp):
+    with fbp.Plan(list(I.uniform_angles(8)), 16, 8, dtype="f32") as plan:
+        with pytest.raises(fbp.FbpError) as ei:
+            fbp.fbp_set_window(plan.handle, 9)
+        assert ei.value.status == fbp.FBP_EINVAL
+        with pytest.raises(fbp.FbpError):
+            fbp.fbp_set_angle_weights(plan.handle, [1.0] * 7 + [float("inf")])
+        with pytest.raises(ValueError):
+            plan.set_angle_weights([1.0] * 3)
+
+
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+def test_metrics_unaligned_views_and_ragged_tails(fbp, oracle, dt):
+    """Pointers that are not 16-byte aligned take the scalar path; lengths that are not a multiple of the
+    vector width leave a tail: both must give the oracle's numbers."""
+    rng = np.random.default_rng(99)
+    x = rng.uniform(0, 1, 100003).astype(_np_dtype(dt))
+    y = rng.uniform(0, 1, 100003).astype(_np_dtype(dt))
+    dx, dy = _dev(x, dt), _dev(y, dt)
+    with fbp.Plan(list(I.uniform_angles(4)), 8, 4, dtype=dt) as plan:
+        for lo, hi in ((0, 100003), (1, 100003), (1, 99999), (3, 4)):
+            got = plan.metrics(dx[lo:hi], dy[lo:hi], 1.0)
+            want = oracle.metrics(x[lo:hi].astype(np.float64), y[lo:hi].astype(np.float64), 1.0)
+            for k in ("mse", "psnr", "ssim", "var_x", "cov_xy"):
+                assert got[k] == pytest.approx(want[k], rel=METRIC_RTOL, abs=1e-18), (lo, hi, k)
