@@ -303,7 +303,17 @@ def run_ours(args):
             mfn()
         m_ms = timed_loop(mfn, 20) / 20
         m_bytes = 4.0 * d_img.numel() * d_img.element_size()
-        extras = {"metrics_ms": m_ms, "metrics_gbs": m_bytes / (m_ms * 1e-3) / 1e9, "metrics_bytes": m_bytes,
+        # fbp_interpolate_stack: the output stack to 4x as many slices (reads <= 2, writes 1 array of the output size)
+        n_out = 4 * B
+        vol = torch.empty((n_out, N, N), dtype=tdt, device="cuda")
+        ifn = lambda: fbp.fbp_interpolate_stack(plan.handle, d_img, B, vol, n_out, stream)  # noqa: E731
+        for _ in range(3):
+            ifn()
+        i_ms = timed_loop(ifn, 20) / 20
+        i_bytes = float(vol.numel() + d_img.numel()) * d_img.element_size()     # algorithmic: read the stack once, write the volume
+        extras = {"stack_interp_ms": i_ms, "stack_interp_gbs": i_bytes / (i_ms * 1e-3) / 1e9, "stack_interp_bytes": i_bytes,
+                  "stack_interp_slices_out": n_out,
+                  "metrics_ms": m_ms, "metrics_gbs": m_bytes / (m_ms * 1e-3) / 1e9, "metrics_bytes": m_bytes,
                   "metrics_launches": 4, "psnr": float(out8[1].item()), "ssim": float(out8[2].item())}
 
     if world > 1:
@@ -374,7 +384,8 @@ def main():
     }
     line["config"]["window"] = args.window
     if r["extras"]:
-        line["extras"] = dict(r["extras"], metrics_hbm_frac=r["extras"]["metrics_gbs"] / float(peaks["hbm_gbs"]))
+        line["extras"] = dict(r["extras"], metrics_hbm_frac=r["extras"]["metrics_gbs"] / float(peaks["hbm_gbs"]),
+                              stack_interp_hbm_frac=r["extras"]["stack_interp_gbs"] / float(peaks["hbm_gbs"]))
     if world == 1 and not args.no_cpu_baseline:
         frac = oracle_fraction(args.config, 15.0, 3)
         g, cores, sample, _ = time_oracle(args.config, frac, reps=3)

@@ -148,6 +148,17 @@ fbp_status fbp_set_window(fbp_plan *plan, fbp_window window);
  */
 fbp_status fbp_set_angle_weights(fbp_plan *plan, const double *h_weights);
 
+/*
+ * fbp_interpolate_stack -- a volume from a stack of reconstructed slices (3-D images
+ * "through the interpolation of a stack of 2D images"; the paper names no rule, LINEAR is the reading
+ * taken, R4).  d_stack [n_in][N][N] in, d_out [n_out][N][N] out (DEVICE, plan dtype, may not
+ * alias).  Output slice m sits at z_m = m (n_in - 1)/(n_out - 1) (z = 0 when n_out = 1):
+ *   k = floor(z_m) clamped to n_in - 2,  t = z_m - k,  out[m] = (1 - t) stack[k] + t stack[k+1];
+ * n_in = 1 copies the slice.  Enqueue-only, one owner thread per output element.
+ */
+fbp_status fbp_interpolate_stack(fbp_plan *plan, const void *d_stack, int n_in, void *d_out, int n_out,
+                                 void *cuda_stream);
+
 /* fbp_destroy -- free the plan, its tables and scratch.  NULL-safe.  Synchronous. */
 void fbp_destroy(fbp_plan *plan);
 

@@ -20,4 +20,5 @@ from .oracle import (  # noqa: F401
     filter_sinogram_window,
     backproject_weighted,
     metrics,
+    interpolate_stack,
 )

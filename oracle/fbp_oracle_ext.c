@@ -182,3 +182,28 @@ void fbp_oracle_metrics(const double *x, const double *y, long n, double max_val
     out[6] = (double)vy;
     out[7] = (double)cxy;
 }
+
+/*
+ * S1: a 3-D volume from a stack of reconstructed 2-D slices by interpolation along the stack axis
+ * ("3D computed tomography images ... through the interpolation of a stack of 2D images";
+ * PAPER.md:222).  The paper does not say which interpolation (its ref [21] is a PDE method that it
+ * does not describe); reading taken (R4): LINEAR interpolation between the two neighbouring
+ * slices, output slice m of n_out at stack coordinate z_m = m (n_in - 1)/(n_out - 1) (z_0 = 0 when
+ * n_out = 1), k = floor(z_m) clamped to n_in - 2, t = z_m - k:
+ *     out[m][p] = (1 - t) in[k][p] + t in[k+1][p]          (n_in = 1: out[m] = in[0]).
+ * `n_pix` = pixels per slice.
+ */
+void fbp_oracle_interpolate_stack(const double *in, int n_in, double *out, int n_out, long n_pix)
+{
+    for (int m = 0; m < n_out; ++m) {
+        double z = n_out > 1 ? (double)m * (double)(n_in - 1) / (double)(n_out - 1) : 0.0;
+        long k = (long)floor(z);
+        if (k > n_in - 2) k = n_in - 2;
+        if (k < 0) k = 0;
+        double t = n_in > 1 ? z - (double)k : 0.0;
+        const double *a = in + (size_t)k * n_pix;
+        const double *b = in + (size_t)(n_in > 1 ? k + 1 : k) * n_pix;
+        double *o = out + (size_t)m * n_pix;
+        for (long p = 0; p < n_pix; ++p) o[p] = (1.0 - t) * a[p] + t * b[p];
+    }
+}

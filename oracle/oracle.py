@@ -68,6 +68,8 @@ def _load():
         lib.fbp_oracle_metrics.argtypes = [_dp, _dp, ctypes.c_long, ctypes.c_double, ctypes.c_double,
                                            ctypes.c_double, _dp]
         lib.fbp_oracle_metrics.restype = None
+        lib.fbp_oracle_interpolate_stack.argtypes = [_dp, ctypes.c_int, _dp, ctypes.c_int, ctypes.c_long]
+        lib.fbp_oracle_interpolate_stack.restype = None
         for fn in ("fbp_oracle_taps", "fbp_oracle_filter", "fbp_oracle_backproject",
                    "fbp_oracle_backproject_pixels", "fbp_oracle_filter_rows",
                    "fbp_oracle_forward_scatter", "fbp_oracle_reconstruct"):
@@ -235,3 +237,13 @@ def metrics(x, y, max_val: float, c1: float | None = None, c2: float | None = No
     lib.fbp_oracle_metrics(_p(a), _p(b), a.size, float(max_val), float(c1), float(c2), _p(out))
     keys = ("mse", "psnr", "ssim", "mu_x", "mu_y", "var_x", "var_y", "cov_xy")
     return dict(zip(keys, (float(v) for v in out)))
+
+
+def interpolate_stack(stack, n_out: int) -> np.ndarray:
+    """Linear interpolation along the stack axis to n_out slices (S1 of fbp_oracle_ext.c)."""
+    lib = _load()
+    a = _f64(stack)
+    assert a.ndim == 3
+    out = np.empty((int(n_out),) + a.shape[1:], dtype=np.float64)
+    lib.fbp_oracle_interpolate_stack(_p(a), a.shape[0], _p(out), int(n_out), a.shape[1] * a.shape[2])
+    return out

@@ -10,7 +10,7 @@ from .binding import (  # noqa: F401
     EXPORTS, FBP_F32, FBP_F64, FBP_OK, FBP_EINVAL, FBP_ENOMEM, FBP_ECUDA, FBP_EUNSUPPORTED,
     FbpError, load_library,
     fbp_create, fbp_filter, fbp_backproject, fbp_reconstruct, fbp_reconstruct_host,
-    fbp_destroy, fbp_last_error, fbp_plan_info, fbp_set_profiling, fbp_get_kernel_ms, fbp_metrics, fbp_set_window, fbp_set_angle_weights, WINDOWS,
+    fbp_destroy, fbp_last_error, fbp_plan_info, fbp_set_profiling, fbp_get_kernel_ms, fbp_metrics, fbp_set_window, fbp_set_angle_weights, WINDOWS, fbp_interpolate_stack,
 )
 from .build import build  # noqa: F401
 
@@ -72,6 +72,17 @@ class Plan:
         b = self._batch(sino, (self.n_angles, self.n_det))
         out = self._empty(sino, (self.image_n, self.image_n)) if out is None else out
         fbp_reconstruct(self.handle, sino, out, b, stream)
+        return out
+
+    def interpolate_stack(self, stack, n_out, out=None, stream=None):
+        """Linear interpolation of a slice stack [n_in][N][N] to n_out slices along the stack axis."""
+        import torch
+        if stack.dtype != self.torch_dtype or not stack.is_cuda or not stack.is_contiguous() or stack.dim() != 3 \
+                or tuple(stack.shape[1:]) != (self.image_n, self.image_n):
+            raise ValueError("expected a contiguous CUDA stack [n_in][N][N] of the plan dtype")
+        if out is None:
+            out = torch.empty((int(n_out), self.image_n, self.image_n), dtype=self.torch_dtype, device=stack.device)
+        fbp_interpolate_stack(self.handle, stack, stack.shape[0], out, n_out, stream)
         return out
 
     def set_window(self, window):

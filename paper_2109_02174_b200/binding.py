@@ -18,7 +18,7 @@ STATUS_NAMES = {0: "FBP_OK", 1: "FBP_EINVAL", 2: "FBP_ENOMEM", 3: "FBP_ECUDA", 4
 EXPORTS = (
     "fbp_create", "fbp_filter", "fbp_backproject", "fbp_reconstruct", "fbp_reconstruct_host",
     "fbp_destroy", "fbp_last_error", "fbp_plan_info", "fbp_set_profiling", "fbp_get_kernel_ms",
-    "fbp_metrics", "fbp_set_window", "fbp_set_angle_weights",
+    "fbp_metrics", "fbp_set_window", "fbp_set_angle_weights", "fbp_interpolate_stack",
 )
 
 PLAN_INFO_FIELDS = (
@@ -61,6 +61,8 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     lib.fbp_set_window.restype = ci
     lib.fbp_set_angle_weights.argtypes = [vp, ctypes.POINTER(cd)]
     lib.fbp_set_angle_weights.restype = ci
+    lib.fbp_interpolate_stack.argtypes = [vp, vp, ci, vp, ci, vp]
+    lib.fbp_interpolate_stack.restype = ci
     lib.fbp_destroy.argtypes = [vp]
     lib.fbp_destroy.restype = None
     lib.fbp_last_error.argtypes = [vp]
@@ -190,3 +192,9 @@ def fbp_set_angle_weights(plan, weights):
         vals = [float(w) for w in weights]
         arr = (ctypes.c_double * max(len(vals), 1))(*vals)
     _check(lib, plan, lib.fbp_set_angle_weights(plan, arr))
+
+
+def fbp_interpolate_stack(plan, d_stack, n_in, d_out, n_out, stream=None):
+    lib = load_library()
+    _check(lib, plan, lib.fbp_interpolate_stack(plan, _ptr(d_stack), int(n_in), _ptr(d_out), int(n_out),
+                                                _stream_handle(stream)))

@@ -19,6 +19,7 @@
 #include "fbp_filter.cuh"
 #include "fbp_filter2.cuh"
 #include "fbp_metrics.cuh"
+#include "fbp_stack.cuh"
 
 namespace {
 
@@ -898,6 +899,30 @@ fbp_status fbp_metrics(fbp_plan* p, const void* d_x, const void* d_y, long long 
     cudaError_t e = p->dtype == FBP_F32 ? launch_metrics<float>(p, d_x, d_y, n, max_val, c1, c2, d_out8, s)
                                         : launch_metrics<double>(p, d_x, d_y, n, max_val, c1, c2, d_out8, s);
     if (e != cudaSuccess) return cuda_fail(p, e, "metrics launch");
+    return FBP_OK;
+}
+
+fbp_status fbp_interpolate_stack(fbp_plan* p, const void* d_stack, int n_in, void* d_out, int n_out, void* stream)
+{
+    if (!p) return FBP_EINVAL;
+    if (!d_stack || !d_out) return fail(p, FBP_EINVAL, "NULL device pointer");
+    if (n_in < 1 || n_out < 1 || n_out > 65535) return fail(p, FBP_EINVAL, "n_in >= 1 and 1 <= n_out <= 65535 required");
+    if (d_stack == d_out) return fail(p, FBP_EINVAL, "fbp_interpolate_stack: input and output may not alias");
+    if ((reinterpret_cast<uintptr_t>(d_stack) | reinterpret_cast<uintptr_t>(d_out)) & (p->esize - 1))
+        return fail(p, FBP_EINVAL, "device pointers must be aligned to the element size");
+    DeviceGuard guard(p->device);
+    const long long n_pix = (long long)p->N * p->N;
+    const long long per_cta = (long long)fbp::kStackThreads * fbp::kStackVecPerThread * (16 / (long long)p->esize);
+    dim3 grid((unsigned)((n_pix + per_cta - 1) / per_cta), (unsigned)n_out);
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (p->dtype == FBP_F32)
+        fbp::interpolate_stack_kernel<float><<<grid, fbp::kStackThreads, 0, s>>>(static_cast<const float*>(d_stack), n_in,
+                                                                               static_cast<float*>(d_out), n_out, n_pix);
+    else
+        fbp::interpolate_stack_kernel<double><<<grid, fbp::kStackThreads, 0, s>>>(static_cast<const double*>(d_stack), n_in,
+                                                                                static_cast<double*>(d_out), n_out, n_pix);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(p, e, "stack interpolation launch");
     return FBP_OK;
 }
 

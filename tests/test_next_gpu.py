@@ -199,3 +199,49 @@ def test_metrics_unaligned_views_and_ragged_tails(fbp, oracle, dt):
             want = oracle.metrics(x[lo:hi].astype(np.float64), y[lo:hi].astype(np.float64), 1.0)
             for k in ("mse", "psnr", "ssim", "var_x", "cov_xy"):
                 assert got[k] == pytest.approx(want[k], rel=METRIC_RTOL, abs=1e-18), (lo, hi, k)
+
+
+# ---- slice stack -> volume (fbp_interpolate_stack) -----------------------------------------------
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+@pytest.mark.parametrize("n,n_in,n_out", [(64, 5, 9), (33, 3, 10), (7, 1, 4), (130, 8, 8), (512, 16, 61), (5, 2, 1)])
+def test_stack_interpolation_matches_oracle(fbp, oracle, dt, n, n_in, n_out):
+    """(1-t) a + t b in the working precision against the fp64 oracle: one rounding of t, one product, one
+    fma => |err| <= 3 ulp of the larger operand (written out: 3 * eps * max|stack|)."""
+    import torch
+    rng = np.random.default_rng(n + n_in + n_out)
+    stack = rng.normal(size=(n_in, n, n)).astype(_np_dtype(dt))
+    want = oracle.interpolate_stack(stack.astype(np.float64), n_out)
+    with fbp.Plan(list(I.uniform_angles(4)), 2 * n, n, dtype=dt) as plan:
+        got = plan.interpolate_stack(_dev(stack, dt), n_out)
+        again = plan.interpolate_stack(_dev(stack, dt), n_out)
+        assert torch.equal(got, again)
+    eps = np.finfo(_np_dtype(dt)).eps
+    assert np.abs(got.cpu().numpy().astype(np.float64) - want).max() <= 3 * eps * np.abs(stack).max()
+    if n_out == n_in:
+        assert np.array_equal(got.cpu().numpy(), stack)             # same grid: t = 0 exactly, identity
+
+
+def test_stack_interpolation_of_reconstructed_slices_and_errors(fbp, oracle):
+    """The paper's use: reconstruct a stack (config-1 geometry, 6 noisy slices), then interpolate it to a volume."""
+    import torch
+    cfg = I.CONFIGS[1]
+    clean = I.config_slice(1)
+    sino = np.stack([I.gaussian_noise(clean * (1.0 + 0.05 * s), 0.01, 4100 + s) for s in range(6)]).astype(np.float32)
+    ang = I.config_angles(1)
+    ref = oracle.interpolate_stack(oracle.reconstruct(sino.astype(np.float64), ang, cfg.image_n), 16)
+    with fbp.Plan(list(ang), cfg.n_det, cfg.image_n, dtype="f32", max_batch=6) as plan:
+        vol = plan.interpolate_stack(plan.reconstruct(_dev(sino, "f32")), 16)
+        _check_image(vol.cpu().numpy(), ref, "f32", "interpolated volume")
+        st = torch.zeros(2, 64, 64, device="cuda")
+        out = torch.full((3, 64, 64), 7.0, device="cuda")
+        for args in ((0, 2, out, 3), (st, 0, out, 3), (st, 2, 0, 3), (st, 2, out, 0), (st, 2, st, 2)):
+            with pytest.raises(fbp.FbpError) as ei:
+                fbp.fbp_interpolate_stack(plan.handle, *args)
+            assert ei.value.status == fbp.FBP_EINVAL
+        torch.cuda.synchronize()
+        assert bool((out == 7.0).all())
+
+
+def test_selfcheck_driver(fbp):
+    from paper_2109_02174_b200 import selfcheck
+    assert selfcheck.main() == 0

@@ -104,3 +104,21 @@ def test_m1_psnr_ssim_closed_forms(oracle):
     assert m["mse"] == pytest.approx(np.mean((x - y) ** 2), rel=1e-13)
     assert m["cov_xy"] == pytest.approx(np.mean((x - x.mean()) * (y - y.mean())), rel=1e-12)
     assert m["var_y"] == pytest.approx(y.var(), rel=1e-13)
+
+
+def test_s1_stack_interpolation_is_numpy_interp_along_z(oracle):
+    """Pins: numpy.interp per pixel column (library routine), endpoints, midpoints, exactness on a linear ramp."""
+    rng = np.random.default_rng(12)
+    stack = rng.normal(size=(5, 3, 4))
+    for n_out in (1, 2, 5, 9, 14):
+        got = oracle.interpolate_stack(stack, n_out)
+        z = np.linspace(0.0, 4.0, n_out) if n_out > 1 else np.zeros(1)
+        for r in range(3):
+            for c in range(4):
+                assert np.allclose(got[:, r, c], np.interp(z, np.arange(5), stack[:, r, c]), rtol=1e-14, atol=1e-15)
+    assert np.array_equal(oracle.interpolate_stack(stack, 5), stack)                    # same grid: identity
+    nine = oracle.interpolate_stack(stack, 9)
+    assert np.array_equal(nine[::2], stack) and np.allclose(nine[1::2], 0.5 * (stack[:-1] + stack[1:]), rtol=1e-15)
+    ramp = np.arange(4.0)[:, None, None] * np.ones((1, 2, 2)) * 3.0 + 1.0              # linear in z: reproduced exactly
+    assert np.allclose(oracle.interpolate_stack(ramp, 10)[:, 0, 0], 1.0 + 3.0 * np.linspace(0, 3, 10), rtol=1e-15)
+    assert np.array_equal(oracle.interpolate_stack(stack[:1], 3), np.repeat(stack[:1], 3, axis=0))
