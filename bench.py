@@ -311,7 +311,16 @@ def run_ours(args):
             ifn()
         i_ms = timed_loop(ifn, 20) / 20
         i_bytes = float(vol.numel() + d_img.numel()) * d_img.element_size()     # algorithmic: read the stack once, write the volume
-        extras = {"stack_interp_ms": i_ms, "stack_interp_gbs": i_bytes / (i_ms * 1e-3) / 1e9, "stack_interp_bytes": i_bytes,
+        # fbp_project: forward projection of the output stack (the adjoint's pixel-angle pairs per second)
+        pb = min(B, 8)
+        d_proj = torch.empty((pb, K, D), dtype=tdt, device="cuda")
+        pfn = lambda: fbp.fbp_project(plan.handle, d_img, d_proj, pb, stream)  # noqa: E731
+        for _ in range(3):
+            pfn()
+        p_ms = timed_loop(pfn, 10) / 10
+        extras = {"project_ms": p_ms, "project_slices": pb,
+                  "project_gupdates_per_s": float(pb) * N * N * K / (p_ms * 1e-3) / 1e9,
+                  "stack_interp_ms": i_ms, "stack_interp_gbs": i_bytes / (i_ms * 1e-3) / 1e9, "stack_interp_bytes": i_bytes,
                   "stack_interp_slices_out": n_out,
                   "metrics_ms": m_ms, "metrics_gbs": m_bytes / (m_ms * 1e-3) / 1e9, "metrics_bytes": m_bytes,
                   "metrics_launches": 4, "psnr": float(out8[1].item()), "ssim": float(out8[2].item())}

@@ -149,6 +149,17 @@ fbp_status fbp_set_window(fbp_plan *plan, fbp_window window);
 fbp_status fbp_set_angle_weights(fbp_plan *plan, const double *h_weights);
 
 /*
+ * fbp_project -- the matched forward projector R = B^T of fbp_backproject WITHOUT its pi/K weight
+ * (rays x cos + y sin = t):
+ *   y[i][j] = sum over pixels (r,c) of max(0, 1 - |u_i(r,c) - j|) * x[r][c],  u_i as in fbp.h's header,
+ * so that <R x, y> = <x, B y> for the unweighted B.  d_image [batch][N][N] in, d_sino [batch][K][D] out
+ * (fully overwritten; may not alias).  A gather with one owner thread per bin and a fixed pixel order:
+ * deterministic, no atomics.  The first call allocates a plan-owned transposed-image scratch
+ * (synchronous); later calls only enqueue.  Angle weights and windows do not apply.
+ */
+fbp_status fbp_project(fbp_plan *plan, const void *d_image, void *d_sino, int batch, void *cuda_stream);
+
+/*
  * fbp_interpolate_stack -- a volume from a stack of reconstructed slices (3-D images
  * "through the interpolation of a stack of 2D images"; the paper names no rule, LINEAR is the reading
  * taken, R4).  d_stack [n_in][N][N] in, d_out [n_out][N][N] out (DEVICE, plan dtype, may not

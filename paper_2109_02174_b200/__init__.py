@@ -10,7 +10,7 @@ from .binding import (  # noqa: F401
     EXPORTS, FBP_F32, FBP_F64, FBP_OK, FBP_EINVAL, FBP_ENOMEM, FBP_ECUDA, FBP_EUNSUPPORTED,
     FbpError, load_library,
     fbp_create, fbp_filter, fbp_backproject, fbp_reconstruct, fbp_reconstruct_host,
-    fbp_destroy, fbp_last_error, fbp_plan_info, fbp_set_profiling, fbp_get_kernel_ms, fbp_metrics, fbp_set_window, fbp_set_angle_weights, WINDOWS, fbp_interpolate_stack,
+    fbp_destroy, fbp_last_error, fbp_plan_info, fbp_set_profiling, fbp_get_kernel_ms, fbp_metrics, fbp_set_window, fbp_set_angle_weights, WINDOWS, fbp_interpolate_stack, fbp_project,
 )
 from .build import build  # noqa: F401
 
@@ -72,6 +72,13 @@ class Plan:
         b = self._batch(sino, (self.n_angles, self.n_det))
         out = self._empty(sino, (self.image_n, self.image_n)) if out is None else out
         fbp_reconstruct(self.handle, sino, out, b, stream)
+        return out
+
+    def project(self, image, out=None, stream=None):
+        """Matched forward projector R = B^T (unweighted): image [batch][N][N] -> sinogram [batch][K][D]."""
+        b = self._batch(image, (self.image_n, self.image_n))
+        out = self._empty(image, (self.n_angles, self.n_det)) if out is None else out
+        fbp_project(self.handle, image, out, b, stream)
         return out
 
     def interpolate_stack(self, stack, n_out, out=None, stream=None):

@@ -18,7 +18,7 @@ STATUS_NAMES = {0: "FBP_OK", 1: "FBP_EINVAL", 2: "FBP_ENOMEM", 3: "FBP_ECUDA", 4
 EXPORTS = (
     "fbp_create", "fbp_filter", "fbp_backproject", "fbp_reconstruct", "fbp_reconstruct_host",
     "fbp_destroy", "fbp_last_error", "fbp_plan_info", "fbp_set_profiling", "fbp_get_kernel_ms",
-    "fbp_metrics", "fbp_set_window", "fbp_set_angle_weights", "fbp_interpolate_stack",
+    "fbp_metrics", "fbp_set_window", "fbp_set_angle_weights", "fbp_interpolate_stack", "fbp_project",
 )
 
 PLAN_INFO_FIELDS = (
@@ -51,7 +51,7 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
     lib.fbp_create.argtypes = [ctypes.POINTER(vp), ci, ci, ctypes.POINTER(cd), cd, ci, cd, ci, ci, ci]
     lib.fbp_create.restype = ci
-    for name in ("fbp_filter", "fbp_backproject", "fbp_reconstruct", "fbp_reconstruct_host"):
+    for name in ("fbp_filter", "fbp_backproject", "fbp_reconstruct", "fbp_reconstruct_host", "fbp_project"):
         fn = getattr(lib, name)
         fn.argtypes = [vp, vp, vp, ci, vp]
         fn.restype = ci
@@ -198,3 +198,8 @@ def fbp_interpolate_stack(plan, d_stack, n_in, d_out, n_out, stream=None):
     lib = load_library()
     _check(lib, plan, lib.fbp_interpolate_stack(plan, _ptr(d_stack), int(n_in), _ptr(d_out), int(n_out),
                                                 _stream_handle(stream)))
+
+
+def fbp_project(plan, d_image, d_sino, batch, stream=None):
+    lib = load_library()
+    _check(lib, plan, lib.fbp_project(plan, _ptr(d_image), _ptr(d_sino), int(batch), _stream_handle(stream)))

@@ -14,7 +14,7 @@ CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(_HERE, "libfbp.so")
 SOURCES = ["fbp.cu"]
-HEADERS = ["fbp_filter.cuh", "fbp_backproject.cuh"]
+HEADERS = sorted(f for f in os.listdir(CSRC) if f.endswith((".cuh", ".h")))   # every header beside fbp.cu
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

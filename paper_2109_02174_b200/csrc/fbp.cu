@@ -20,6 +20,7 @@
 #include "fbp_filter2.cuh"
 #include "fbp_metrics.cuh"
 #include "fbp_stack.cuh"
+#include "fbp_project.cuh"
 
 namespace {
 
@@ -76,6 +77,7 @@ struct fbp_plan {
     fbp::Filter2Params f2d{};
     void* d_ud = nullptr;       // [2][tab_len] dtype: UA | UB of the dense table, U[j] = H[2 a_tot - j]
     void* d_rhod = nullptr;     // [D] dtype
+    void* d_xt = nullptr;       // [max_batch][N][N] dtype: transposed image for fbp_project (allocated on first use)
     void* d_wrow = nullptr;     // [K] dtype: angle weight / (pi/K) (fbp_set_angle_weights); NULL = uniform
 
     double* d_mscratch = nullptr;   // fbp_metrics: [kMetricGrid][3] CTA partials, then mid[3]
@@ -787,7 +789,7 @@ void fbp_destroy(fbp_plan* p)
         DeviceGuard guard(p->device);
         cudaFree(p->d_cs2); cudaFree(p->d_taps); cudaFree(p->d_rho); cudaFree(p->d_ent); cudaFree(p->d_part); cudaFree(p->d_tickets);
         cudaFree(p->d_hsino); cudaFree(p->d_himg); cudaFree(p->d_u); cudaFree(p->d_rho2); cudaFree(p->d_mscratch);
-        cudaFree(p->d_ud); cudaFree(p->d_rhod); cudaFree(p->d_wrow);
+        cudaFree(p->d_ud); cudaFree(p->d_rhod); cudaFree(p->d_wrow); cudaFree(p->d_xt);
         for (int i = 0; i < 4; ++i) if (p->ev[i]) cudaEventDestroy(p->ev[i]);
         if (p->st_f) { cudaStreamSynchronize(p->st_f); cudaStreamDestroy(p->st_f); }
         for (int i = 0; i < 2; ++i) if (p->st_b[i]) { cudaStreamSynchronize(p->st_b[i]); cudaStreamDestroy(p->st_b[i]); }
@@ -899,6 +901,31 @@ fbp_status fbp_metrics(fbp_plan* p, const void* d_x, const void* d_y, long long 
     cudaError_t e = p->dtype == FBP_F32 ? launch_metrics<float>(p, d_x, d_y, n, max_val, c1, c2, d_out8, s)
                                         : launch_metrics<double>(p, d_x, d_y, n, max_val, c1, c2, d_out8, s);
     if (e != cudaSuccess) return cuda_fail(p, e, "metrics launch");
+    return FBP_OK;
+}
+
+fbp_status fbp_project(fbp_plan* p, const void* d_image, void* d_sino, int batch, void* stream)
+{
+    fbp_status st = check_call(p, d_image, d_sino, batch);
+    if (st != FBP_OK) return st;
+    if (d_image == d_sino) return fail(p, FBP_EINVAL, "fbp_project: input and output may not alias");
+    DeviceGuard guard(p->device);
+    if (!p->d_xt) FBP_CUDA(p, cudaMalloc(&p->d_xt, p->esize * (size_t)p->max_batch * p->N * p->N));
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    fbp::ProjParams prm{p->K, p->D, p->N, 0.5 * (p->N - 1), 0.5 * (p->D - 1)};
+    const dim3 tgrid((p->N + 31) / 32, (p->N + 31) / 32, batch), tblock(32, 8);
+    const dim3 pgrid((p->D + 127) / 128, p->K, batch);
+    if (p->dtype == FBP_F32) {
+        fbp::transpose_kernel<float><<<tgrid, tblock, 0, s>>>(static_cast<const float*>(d_image), static_cast<float*>(p->d_xt), p->N);
+        fbp::project_kernel<float><<<pgrid, 128, 0, s>>>(static_cast<const float*>(d_image), static_cast<const float*>(p->d_xt),
+                                                        static_cast<float*>(d_sino), p->d_cs2, prm);
+    } else {
+        fbp::transpose_kernel<double><<<tgrid, tblock, 0, s>>>(static_cast<const double*>(d_image), static_cast<double*>(p->d_xt), p->N);
+        fbp::project_kernel<double><<<pgrid, 128, 0, s>>>(static_cast<const double*>(d_image), static_cast<const double*>(p->d_xt),
+                                                         static_cast<double*>(d_sino), p->d_cs2, prm);
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(p, e, "projector launch");
     return FBP_OK;
 }
 
