@@ -188,7 +188,7 @@ const char *fbp_last_error(const fbp_plan *plan);
  *   [6] back-projection CTAs per slice   [7] back-projection threads per CTA
  *   [8] back-projection dynamic shared memory bytes per CTA
  *   [9] filter outputs per thread   [10] filter threads per CTA   [11] filter input slices per row (SB)
- *   [12] filter dynamic shared memory bytes per CTA   [13] kernels launched by fbp_reconstruct
+ *   [12] filter dynamic shared memory bytes per CTA   [13] kernels launched by fbp_reconstruct at batch = max_batch
  */
 int fbp_plan_info(const fbp_plan *plan, int *out, int n);
 

@@ -1021,11 +1021,20 @@ fbp_status fbp_set_angle_weights(fbp_plan* p, const double* h_weights)
 int fbp_plan_info(const fbp_plan* p, int* out, int n)
 {
     if (!p) return 0;
+    // kernels launched by fbp_reconstruct at batch = max_batch: filter + back-projection, per slice group when
+    // the batch pipeline is on
+    int launches = 2;
+    if (use_pipeline(p, p->max_batch)) {
+        int group = p->pipe_group > 0 ? p->pipe_group : (p->max_batch + 3) / 4;
+        const int min_group = (p->max_batch + fbp_plan::kMaxGroups - 1) / fbp_plan::kMaxGroups;
+        if (group < min_group) group = min_group;
+        launches = 2 * ((p->max_batch + group - 1) / group);
+    }
     const int v[14] = {p->bp_tw, p->bp_th, p->bp_r, p->bp_splits, p->bp_chunk, p->bp_seg,
                        p->bp.tiles_x * p->bp.tiles_y * p->bp_splits, p->bp_threads, p->bp_smem,
                        p->filter_v == 2 ? 2 * p->f2_r : p->f_r, p->filter_v == 2 ? p->f2_threads : p->f_threads,
                        p->filter_v == 2 ? p->f2.n_sb : p->fp.n_sb, p->filter_v == 2 ? p->f2_smem : p->f_smem,
-                       2};
+                       launches};
     if (out) for (int i = 0; i < n && i < 14; ++i) out[i] = v[i];
     return 14;
 }
