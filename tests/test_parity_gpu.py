@@ -307,3 +307,38 @@ def test_batch_pipeline_is_bit_identical_to_sequential(fbp, oracle, dt, group, m
     assert torch.equal(again, want[:11])
     ref = oracle.reconstruct(sino[3].astype(np.float64), ang, n)
     check_image(got[3].cpu().numpy(), ref, dt, "pipeline slice 3")
+
+
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+def test_first_generation_filter_kernel_still_matches(fbp, oracle, dt, monkeypatch):
+    """FBP_FILTER_V=1 selects the one-parity filter kernel kept as the fallback for rows that do not fit the
+    paired kernel's shared-memory layout; it must meet the same tolerances."""
+    monkeypatch.setenv("FBP_FILTER_V", "1")
+    cfg = I.CONFIGS[2]
+    run_case(fbp, oracle, I.config_sinogram(2), I.config_angles(2), cfg.image_n, dt, what="cfg2 filter v1")
+    run_case(fbp, oracle, I.random_sinogram(31, 2, 9, 70), I.uniform_angles(9), 45, dt, 0.5, 0.5, what="odd filter v1")
+
+
+def test_long_rows_and_many_angles(fbp, oracle):
+    """Edge of the supported range in one direction each: a 4099-bin row (filter blocks, guards) on a small image,
+    and 4000 angles on a small image (chunking, records); sampled against the oracle."""
+    dd, k, n = 4099, 6, 96
+    sino = I.random_sinogram(77, 1, k, dd).astype(np.float32)
+    ang = I.uniform_angles(k)
+    plan = fbp.Plan(list(ang), dd, n, dtype="f32")
+    try:
+        q = plan.filter(_to_dev(sino, "f32")).cpu().numpy()
+        check_filter(q, oracle.filter_sinogram(sino.astype(np.float64)), "f32", "long row", np.abs(sino).max())
+        f = plan.reconstruct(_to_dev(sino, "f32")).cpu().numpy()
+        check_image(f, oracle.reconstruct(sino.astype(np.float64), ang, n), "f32", "long row recon")
+    finally:
+        plan.close()
+    dd, k, n = 61, 4000, 40
+    sino = I.random_sinogram(78, 1, k, dd)
+    ang = np.sort(np.random.default_rng(5).uniform(0, 2 * math.pi, k))
+    plan = fbp.Plan(list(ang), dd, n, dtype="f64")
+    try:
+        f = plan.reconstruct(_to_dev(sino, "f64")).cpu().numpy()
+        check_image(f, oracle.reconstruct(sino, ang, n), "f64", "many angles")
+    finally:
+        plan.close()
