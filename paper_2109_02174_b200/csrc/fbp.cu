@@ -50,6 +50,7 @@ struct fbp_plan {
     void* d_taps = nullptr;     // [tab_len] dtype: G[q + tab_off] = g[q]
     void* d_rho = nullptr;      // [D] dtype: conditioning term of the filter (fbp_filter.cuh)
     void* d_ent = nullptr;      // [max_batch][K][ent_pitch] BpEntry: back-projector operands
+    void* d_recs = nullptr;     // [tiles][K] AngleRec: per (tile, angle) records of the back-projector (or NULL)
     void* d_part = nullptr;     // [S][max_batch][N][N] partial images when S > 1
     int* d_tickets = nullptr;   // [max_batch][tiles] arrival counters when S > 1 (self re-arming)
     void* d_hsino = nullptr;    // host-path staging (lazy)
@@ -757,6 +758,45 @@ fbp_status fbp_create(fbp_plan** out, int n_angles, int n_det, const double* ang
     FBP_TRY(cudaMemcpy(p->d_u, usrc, p->esize * 2 * (size_t)tl2, cudaMemcpyHostToDevice));
     FBP_TRY(cudaMalloc(&p->d_rho2, p->esize * (size_t)n_det));
     FBP_TRY(cudaMemcpy(p->d_rho2, r2src, p->esize * (size_t)n_det, cudaMemcpyHostToDevice));
+    // Optional (FBP_BP_RECS=1): back-projector records per (tile, angle) computed here in fp64 with the formulas of
+    // the kernel's own path, so that the producer warp only copies them.  Measured on B200: no change in fp32
+    // (the producer is not the limiter: cfg3 33.2 us either way) and slower in fp64 (32-byte records: 56 -> 73 us),
+    // so it is off by default.
+    {
+        const size_t n_tiles = (size_t)p->bp.tiles_x * p->bp.tiles_y;
+        const size_t bytes = n_tiles * n_angles * 4 * p->esize;
+        if (bytes <= ((size_t)128 << 20) && env_int("FBP_BP_RECS", 0)) {
+            std::vector<unsigned char> host(bytes);
+            const int TH = p->bp_th, L = p->bp_seg;
+            for (size_t t = 0; t < n_tiles; ++t) {
+                const int ty = (int)(t / p->bp.tiles_x), tx = (int)(t % p->bp.tiles_x);
+                const double x0 = (double)(tx * 32) - p->bp.c_n, y0 = (double)(ty * TH) - p->bp.c_n;
+                for (int i = 0; i < n_angles; ++i) {
+                    const double cx = cs[2 * i], sy = cs[2 * i + 1];
+                    const double ub = x0 * cx + y0 * sy + p->bp.c_d;
+                    const double umin = ub + std::fmin(0.0, 31.0 * cx) + std::fmin(0.0, (double)(TH - 1) * sy);
+                    const double fl = std::floor(umin) - 1.0;
+                    const bool on = fl >= -(double)p->bp.ent_guard && fl <= (double)(p->bp.ent_pitch - p->bp.ent_guard - L);
+                    const int off = on ? (int)fl + p->bp.ent_guard : 0;
+                    const size_t idx = t * n_angles + i;
+                    if (dtype == FBP_F32) {
+                        fbp::AngleRec<float> rc;
+                        rc.c = on ? (float)cx : 0.f; rc.s = on ? (float)sy : 0.f; rc.b = on ? (float)(ub - fl - 0.5) : 1.f;
+                        rc.pad = fbp::RecOffset<float>::put(off);
+                        std::memcpy(host.data() + idx * sizeof(rc), &rc, sizeof(rc));
+                    } else {
+                        fbp::AngleRec<double> rc;
+                        rc.c = on ? cx : 0.0; rc.s = on ? sy : 0.0; rc.b = on ? ub - fl - 0.5 : 1.0;
+                        rc.pad = fbp::RecOffset<double>::put(off);
+                        std::memcpy(host.data() + idx * sizeof(rc), &rc, sizeof(rc));
+                    }
+                }
+            }
+            FBP_TRY(cudaMalloc(&p->d_recs, bytes));
+            FBP_TRY(cudaMemcpy(p->d_recs, host.data(), bytes, cudaMemcpyHostToDevice));
+        }
+        p->bp.recs = p->d_recs;
+    }
     FBP_TRY(cudaMalloc(&p->d_ent, 4 * p->esize * (size_t)max_batch * n_angles * p->bp.ent_pitch));
     if (p->bp_splits > 1) {
         const size_t nt = (size_t)max_batch * p->bp.tiles_x * p->bp.tiles_y;
@@ -789,7 +829,7 @@ void fbp_destroy(fbp_plan* p)
         DeviceGuard guard(p->device);
         cudaFree(p->d_cs2); cudaFree(p->d_taps); cudaFree(p->d_rho); cudaFree(p->d_ent); cudaFree(p->d_part); cudaFree(p->d_tickets);
         cudaFree(p->d_hsino); cudaFree(p->d_himg); cudaFree(p->d_u); cudaFree(p->d_rho2); cudaFree(p->d_mscratch);
-        cudaFree(p->d_ud); cudaFree(p->d_rhod); cudaFree(p->d_wrow); cudaFree(p->d_xt);
+        cudaFree(p->d_recs); cudaFree(p->d_ud); cudaFree(p->d_rhod); cudaFree(p->d_wrow); cudaFree(p->d_xt);
         for (int i = 0; i < 4; ++i) if (p->ev[i]) cudaEventDestroy(p->ev[i]);
         if (p->st_f) { cudaStreamSynchronize(p->st_f); cudaStreamDestroy(p->st_f); }
         for (int i = 0; i < 2; ++i) if (p->st_b[i]) { cudaStreamSynchronize(p->st_b[i]); cudaStreamDestroy(p->st_b[i]); }

@@ -54,6 +54,7 @@ struct BpParams {
     int ent_pitch, ent_guard;
     double c_n, c_d;     // (N-1)/2, (D-1)/2
     double scale;        // pi / K
+    const void* recs;    // [tiles][K] AngleRec<T> precomputed by fbp_create (pad = entry offset), or NULL
 };
 
 template <typename T> struct Magic;
@@ -69,6 +70,16 @@ template <> struct Magic<double> {
 };
 
 template <typename T> struct alignas(4 * sizeof(T)) AngleRec { T c, s, b, pad; };
+// the entry offset of a precomputed record travels in `pad` as raw integer bits
+template <typename T> struct RecOffset;
+template <> struct RecOffset<float> {
+    __host__ __device__ static float put(int off) { union { int i; float f; } u; u.i = off; return u.f; }
+    __device__ static long long get(float pad) { return (long long)__float_as_int(pad); }
+};
+template <> struct RecOffset<double> {
+    __host__ __device__ static double put(int off) { union { long long i; double f; } u; u.i = off; return u.f; }
+    __device__ static long long get(double pad) { return __double_as_longlong(pad); }
+};
 
 // ---- PTX wrappers: shared-space addresses, mbarrier, TMA 1-D bulk copy ----------------
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -225,25 +236,31 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
             const int na = min(prm.chunk, a_end - a0);
             const unsigned bar = bar_full + 8u * st;
             for (int a = lane; a < na; a += 32) {
-                const double2 cs = cs2[a0 + a];
-                const double ub = x0 * cs.x + y0 * cs.y + prm.c_d;
-                const double umin = ub + fmin(0.0, 31.0 * cs.x) + fmin(0.0, (double)(TH - 1) * cs.y);
-                const double fl = floor(umin) - 1.0;
                 AngleRec<T> rc;
-                long long j0;
-                // the window [j0, j0+L) must lie inside the guarded row [-guard, pitch-guard)
-                if (fl >= -(double)prm.ent_guard && fl <= (double)(prm.ent_pitch - prm.ent_guard - L)) {
-                    j0 = (long long)fl;
-                    rc.c = (T)cs.x; rc.s = (T)cs.y; rc.b = (T)(ub - fl - 0.5);
+                long long off;            // first staged entry of this angle's row, in entries from the row start
+                if (prm.recs) {
+                    // records precomputed on the host (same fp64 formulas as below): the producer only copies
+                    rc = static_cast<const AngleRec<T>*>(prm.recs)[(size_t)tile * K + a0 + a];
+                    off = RecOffset<T>::get(rc.pad);
                 } else {
-                    // the tile projects entirely off the detector at this angle: stage the
-                    // all-zero left guard and pin every pixel to entry 1 of it
-                    j0 = -(long long)prm.ent_guard;
-                    rc.c = T(0); rc.s = T(0); rc.b = T(1);
+                    const double2 cs = cs2[a0 + a];
+                    const double ub = x0 * cs.x + y0 * cs.y + prm.c_d;
+                    const double umin = ub + fmin(0.0, 31.0 * cs.x) + fmin(0.0, (double)(TH - 1) * cs.y);
+                    const double fl = floor(umin) - 1.0;
+                    // the window [j0, j0+L) must lie inside the guarded row [-guard, pitch-guard)
+                    if (fl >= -(double)prm.ent_guard && fl <= (double)(prm.ent_pitch - prm.ent_guard - L)) {
+                        off = (long long)fl + prm.ent_guard;
+                        rc.c = (T)cs.x; rc.s = (T)cs.y; rc.b = (T)(ub - fl - 0.5);
+                    } else {
+                        // the tile projects entirely off the detector at this angle: stage the
+                        // all-zero left guard and pin every pixel to entry 1 of it
+                        off = 0;
+                        rc.c = T(0); rc.s = T(0); rc.b = T(1);
+                    }
+                    rc.pad = T(0);
                 }
-                rc.pad = T(0);
                 rec[st * prm.chunk + a] = rc;
-                const uint4* src = Eb + (size_t)(a0 + a) * NP * prm.ent_pitch + (j0 + prm.ent_guard);
+                const uint4* src = Eb + (size_t)(a0 + a) * NP * prm.ent_pitch + off;
 #pragma unroll
                 for (int pl = 0; pl < NP; ++pl)
                     tma_load_1d(seg + st * stage_stride + pl * plane_stride + (unsigned)(a * L * 16),
