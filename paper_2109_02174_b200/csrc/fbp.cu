@@ -78,7 +78,7 @@ struct fbp_plan {
     fbp::Filter2Params f2d{};
     void* d_ud = nullptr;       // [2][tab_len] dtype: UA | UB of the dense table, U[j] = H[2 a_tot - j]
     void* d_rhod = nullptr;     // [D] dtype
-    void* d_xt = nullptr;       // [max_batch][N][N] dtype: transposed image for fbp_project (allocated on first use)
+    void* d_xt = nullptr;       // 2 x [max_batch][N][N + 2 pad] dtype: padded image and padded transpose for fbp_project
     void* d_wrow = nullptr;     // [K] dtype: angle weight / (pi/K) (fbp_set_angle_weights); NULL = uniform
 
     double* d_mscratch = nullptr;   // fbp_metrics: [kMetricGrid][3] CTA partials, then mid[3]
@@ -950,19 +950,25 @@ fbp_status fbp_project(fbp_plan* p, const void* d_image, void* d_sino, int batch
     if (st != FBP_OK) return st;
     if (d_image == d_sino) return fail(p, FBP_EINVAL, "fbp_project: input and output may not alias");
     DeviceGuard guard(p->device);
-    if (!p->d_xt) FBP_CUDA(p, cudaMalloc(&p->d_xt, p->esize * (size_t)p->max_batch * p->N * p->N));
+    // zero pad of the staged lines: the widest run is 2 E + 1 pixels, E <= ceil(sqrt(2) d/pix + 1/2) - 1
+    const int e_max = (int)std::ceil(std::sqrt(2.0) * p->d / p->pix + 0.5) - 1;
+    const int pad = round_up(2 * e_max + 2, 4);            // round(p*) is clamped to [-(E+1), N+E], the run adds +-E
+    const size_t plane = (size_t)p->N * (p->N + 2 * pad);
+    if (!p->d_xt) FBP_CUDA(p, cudaMalloc(&p->d_xt, p->esize * 2 * (size_t)p->max_batch * plane));
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    fbp::ProjParams prm{p->K, p->D, p->N, 0.5 * (p->N - 1), 0.5 * (p->D - 1)};
+    fbp::ProjParams prm{p->K, p->D, p->N, pad, 0.5 * (p->N - 1), 0.5 * (p->D - 1)};
     const dim3 tgrid((p->N + 31) / 32, (p->N + 31) / 32, batch), tblock(32, 8);
     const dim3 pgrid((p->D + 127) / 128, p->K, batch);
     if (p->dtype == FBP_F32) {
-        fbp::transpose_kernel<float><<<tgrid, tblock, 0, s>>>(static_cast<const float*>(d_image), static_cast<float*>(p->d_xt), p->N);
-        fbp::project_kernel<float><<<pgrid, 128, 0, s>>>(static_cast<const float*>(d_image), static_cast<const float*>(p->d_xt),
-                                                        static_cast<float*>(d_sino), p->d_cs2, prm);
+        float* xp = static_cast<float*>(p->d_xt);
+        float* xtp = xp + (size_t)p->max_batch * plane;
+        fbp::stage_image_kernel<float><<<tgrid, tblock, 0, s>>>(static_cast<const float*>(d_image), xp, xtp, p->N, pad);
+        fbp::project_kernel<float><<<pgrid, 128, 0, s>>>(xp, xtp, static_cast<float*>(d_sino), p->d_cs2, prm);
     } else {
-        fbp::transpose_kernel<double><<<tgrid, tblock, 0, s>>>(static_cast<const double*>(d_image), static_cast<double*>(p->d_xt), p->N);
-        fbp::project_kernel<double><<<pgrid, 128, 0, s>>>(static_cast<const double*>(d_image), static_cast<const double*>(p->d_xt),
-                                                         static_cast<double*>(d_sino), p->d_cs2, prm);
+        double* xp = static_cast<double*>(p->d_xt);
+        double* xtp = xp + (size_t)p->max_batch * plane;
+        fbp::stage_image_kernel<double><<<tgrid, tblock, 0, s>>>(static_cast<const double*>(d_image), xp, xtp, p->N, pad);
+        fbp::project_kernel<double><<<pgrid, 128, 0, s>>>(xp, xtp, static_cast<double*>(d_sino), p->d_cs2, prm);
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(p, e, "projector launch");
