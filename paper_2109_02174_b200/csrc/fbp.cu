@@ -27,6 +27,7 @@ namespace {
 constexpr double kPi = 3.14159265358979323846264338327950288;
 constexpr int kNumSm = 148;  // B200
 constexpr int kMetricGrid = 8 * kNumSm;
+constexpr int kTabCopies = 1;    // replicas of the filter tap table in global memory; 16 measured no faster than 1 (no L2 hot spot)
 
 thread_local std::string g_create_error;
 
@@ -450,11 +451,16 @@ cudaError_t launch_filter2_r(fbp_plan* p, const void* sino, void* filt, void* en
         if (per_sm < 1) return cudaErrorLaunchOutOfResources;
         cap = per_sm * kNumSm;
     }
-    const int grid = f.n_rows < cap ? f.n_rows : cap;
+    // A whole number of CTAs per SM: with 360 rows on 148 SMs the 64 CTAs of a third, partial round were starved
+    // of issue slots by the two FMA-bound CTAs already computing on their SM (measured with %globaltimer: their
+    // tables "landed" 4.6 us late and the kernel ended at 10.5 us); with 296 persistent CTAs, 64 of which take a
+    // second row, every CTA on an SM reaches its compute phase together.
+    int grid = f.n_rows < cap ? f.n_rows : cap;
+    if (grid > kNumSm && env_int("FBP_FILTER_WHOLE_WAVES", 1)) grid -= grid % kNumSm;
     kern<<<grid, threads, smem, st>>>(static_cast<const T*>(sino), static_cast<T*>(filt), static_cast<uint4*>(ent),
                                       static_cast<const T*>(DENSE ? p->d_ud : p->d_u),
                                       static_cast<const T*>(DENSE ? p->d_rhod : p->d_rho2),
-                                      static_cast<const T*>(p->d_wrow), p->K, f, (T)(1.0 / p->d));
+                                      static_cast<const T*>(p->d_wrow), p->K, f, (T)(1.0 / p->d), kTabCopies);
     return cudaGetLastError();
 }
 
@@ -754,8 +760,10 @@ fbp_status fbp_create(fbp_plan** out, int n_angles, int n_det, const double* ang
     FBP_TRY(cudaMemcpy(p->d_taps, gsrc, p->esize * (size_t)tl, cudaMemcpyHostToDevice));
     FBP_TRY(cudaMalloc(&p->d_rho, p->esize * (size_t)n_det));
     FBP_TRY(cudaMemcpy(p->d_rho, rsrc, p->esize * (size_t)n_det, cudaMemcpyHostToDevice));
-    FBP_TRY(cudaMalloc(&p->d_u, p->esize * 2 * (size_t)tl2));
-    FBP_TRY(cudaMemcpy(p->d_u, usrc, p->esize * 2 * (size_t)tl2, cudaMemcpyHostToDevice));
+    FBP_TRY(cudaMalloc(&p->d_u, p->esize * 2 * (size_t)tl2 * kTabCopies));
+    for (int c = 0; c < kTabCopies; ++c)
+        FBP_TRY(cudaMemcpy(static_cast<char*>(p->d_u) + (size_t)c * p->esize * 2 * tl2, usrc, p->esize * 2 * (size_t)tl2,
+                           cudaMemcpyHostToDevice));
     FBP_TRY(cudaMalloc(&p->d_rho2, p->esize * (size_t)n_det));
     FBP_TRY(cudaMemcpy(p->d_rho2, r2src, p->esize * (size_t)n_det, cudaMemcpyHostToDevice));
     // Optional (FBP_BP_RECS=1): back-projector records per (tile, angle) computed here in fp64 with the formulas of
@@ -1032,9 +1040,11 @@ fbp_status fbp_set_window(fbp_plan* p, fbp_window window)
         u32.assign(u64.begin(), u64.end()); usrc = u32.data();
         rho32.assign(rho64.begin(), rho64.end()); rsrc = rho32.data();
     }
-    if (!p->d_ud) FBP_CUDA(p, cudaMalloc(&p->d_ud, p->esize * 2 * (size_t)tl));
+    if (!p->d_ud) FBP_CUDA(p, cudaMalloc(&p->d_ud, p->esize * 2 * (size_t)tl * kTabCopies));
     if (!p->d_rhod) FBP_CUDA(p, cudaMalloc(&p->d_rhod, p->esize * (size_t)D));
-    FBP_CUDA(p, cudaMemcpy(p->d_ud, usrc, p->esize * 2 * (size_t)tl, cudaMemcpyHostToDevice));
+    for (int c = 0; c < kTabCopies; ++c)
+        FBP_CUDA(p, cudaMemcpy(static_cast<char*>(p->d_ud) + (size_t)c * p->esize * 2 * tl, usrc, p->esize * 2 * (size_t)tl,
+                               cudaMemcpyHostToDevice));
     FBP_CUDA(p, cudaMemcpy(p->d_rhod, rsrc, p->esize * (size_t)D, cudaMemcpyHostToDevice));
     p->window = (int)window;
     return FBP_OK;
@@ -1113,3 +1123,10 @@ fbp_status fbp_get_kernel_ms(fbp_plan* p, float* filter_ms, float* backproject_m
 }
 
 }  // extern "C"
+
+#ifdef FBP_TRACE
+extern "C" int fbp_debug_read_trace(unsigned long long* out, int n)
+{
+    return (int)cudaMemcpyFromSymbol(out, fbp::g_trace, sizeof(unsigned long long) * (size_t)n);
+}
+#endif

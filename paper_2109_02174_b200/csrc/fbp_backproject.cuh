@@ -44,6 +44,12 @@
 
 namespace fbp {
 
+#ifdef FBP_TRACE
+#define FBP_BP_MARK(slot) do { if (threadIdx.x == 0 && blockIdx.x < 4096) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_trace[blockIdx.x * 16 + 8 + (slot)] = t_; } } while (0)
+#else
+#define FBP_BP_MARK(slot) do { } while (0)
+#endif
+
 struct BpParams {
     int n_angles, n_det, image_n;
     int half_rows;       // ceil(N/2): rows of the primary (top) half
@@ -193,6 +199,7 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
     const unsigned seg = smem_u32(seg_ptr);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    FBP_BP_MARK(0);
     const bool producer = warp == NW;
     const int wy = warp % WY, wa = producer ? WA : warp / WY;
     const int tile = blockIdx.x;
@@ -219,6 +226,7 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
     // E.  Every thread blocks here (consumers would otherwise spin on their mbarriers and take issue
     // slots from that kernel); a no-op when launched without the attribute.
     asm volatile("griddepcontrol.wait;" ::: "memory");
+    FBP_BP_MARK(1);
 
     PairAcc<T> acc[R];
 #pragma unroll
@@ -279,6 +287,7 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
             const int st = k % NS;
             const int na = min(prm.chunk, a_end - (a_begin + k * prm.chunk));
             mbar_wait(bar_full + 8u * st, (unsigned)((k / NS) & 1));  // chunk k has landed
+            if (k == 0) FBP_BP_MARK(2);
             const AngleRec<T>* rk = rec + st * prm.chunk;
             const unsigned segk = seg + st * stage_stride - Magic<T>::kBits * 16u;  // bits(M) folded in
 #pragma unroll 2
@@ -299,6 +308,7 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
         }
     }
 
+    FBP_BP_MARK(3);
     // ---- in-CTA reduction over the WA angle groups, fixed order g = 0..WA-1 ----
     T va[R], vb[R];
 #pragma unroll
@@ -343,6 +353,7 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
             if (ok_a(r)) img[base_a + (long long)r * N] = va[r] * sc;
             if (ok_b(r)) img[base_b - (long long)r * N] = vb[r] * sc;
         }
+        FBP_BP_MARK(4);
         return;
     }
 

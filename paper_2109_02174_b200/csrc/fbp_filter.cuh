@@ -31,6 +31,14 @@
 
 namespace fbp {
 
+#ifdef FBP_TRACE   // phase timestamps for _work experiments (never defined in the product build)
+__device__ unsigned long long g_trace[16 * 4096];
+__device__ __forceinline__ unsigned long long trace_now()
+{
+    unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t;
+}
+#endif
+
 struct FilterParams {
     int n_rows;            // batch * K
     int n_det;             // D

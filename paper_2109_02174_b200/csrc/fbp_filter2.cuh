@@ -91,7 +91,14 @@ template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile(
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
-// U_gmem: [2][tab_len] = UA | UB (see above), U[j] = g[a_tot - 1 - j].  rho: [D].
+#ifdef FBP_TRACE
+#define FBP_TRACE_MARK(slot) do { if (threadIdx.x == 0 && blockIdx.x < 4096) g_trace[blockIdx.x * 16 + (slot)] = trace_now(); } while (0)
+#else
+#define FBP_TRACE_MARK(slot) do { } while (0)
+#endif
+
+// U_gmem: [tab_copies][2][tab_len] = UA | UB (see above), U[j] = g[a_tot - 1 - j]; CTAs read replica
+// blockIdx % tab_copies (every CTA stages the same table at the same moment: one copy is an L2 hot spot).  rho: [D].
 // Block = n_ob * n_sb warps.  Grid <= number of co-resident CTAs (persistent).
 //
 // DENSE = true is the general form for apodised windows (every tap non-zero; SURVEY.md 8(f) row 1,
@@ -104,7 +111,7 @@ template <typename T, int R, bool DENSE>
 __global__ void __launch_bounds__(512)
 filter2_kernel(const T* __restrict__ P, T* __restrict__ Q, uint4* __restrict__ E,
                const T* __restrict__ U_gmem, const T* __restrict__ rho, const T* __restrict__ wrow,
-               int n_angles, Filter2Params prm, T inv_d)
+               int n_angles, Filter2Params prm, T inv_d, int tab_copies)
 {
     static_assert(DENSE ? (R % 2 == 1) : (R % 4 == 2), "lane stride (R or 2R words) must be 2 mod 4: conflict-free pair loads");
     using P2 = Pair2<T>;
@@ -121,6 +128,7 @@ filter2_kernel(const T* __restrict__ P, T* __restrict__ Q, uint4* __restrict__ E
     T* rho_s = yz + prm.ent_pitch + 2;
 
     pdl_launch_dependents();   // every CTA of this grid is resident: dependents may take what is left
+    FBP_TRACE_MARK(0);
 
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int D = prm.n_det;
@@ -128,15 +136,23 @@ filter2_kernel(const T* __restrict__ P, T* __restrict__ Q, uint4* __restrict__ E
     const int sb = warp % prm.n_sb, ob = warp / prm.n_sb;
 
     // ---- once per CTA: tap tables, zero padding of both input buffers, first row ----
-    for (int i = tid * (16 / (int)sizeof(T)); i < 2 * prm.tab_len; i += nthr * (16 / (int)sizeof(T)))
-        cp_async<16>(UA + i, U_gmem + i);
-    for (int k = tid; k < D; k += nthr) cp_async<(int)sizeof(T)>(rho_s + k, rho + k);
+    {
+        const T* Ug = U_gmem + (size_t)(blockIdx.x % tab_copies) * 2 * prm.tab_len;
+        for (int i = tid * (16 / (int)sizeof(T)); i < 2 * prm.tab_len; i += nthr * (16 / (int)sizeof(T)))
+            cp_async<16>(UA + i, Ug + i);
+    }
     for (int k = D + tid; k < x_len; k += nthr) { X0[k] = T(0); X0[x_len + k] = T(0); }
+#ifdef FBP_TRACE
+    cp_async_commit();         // tables in their own group, to time them apart from the row
+#endif
     int row = blockIdx.x;
     if (row < prm.n_rows) {
         const T* prow = P + (size_t)row * D;
         for (int k = tid; k < D; k += nthr) cp_async<(int)sizeof(T)>(X0 + k, prow + k);
     }
+    cp_async_commit();
+    // the conditioning term is needed only by the reduction: its own group, waited for there
+    for (int k = tid; k < D; k += nthr) cp_async<(int)sizeof(T)>(rho_s + k, rho + k);
     cp_async_commit();
 
     // per-thread constants
@@ -161,8 +177,13 @@ filter2_kernel(const T* __restrict__ P, T* __restrict__ Q, uint4* __restrict__ E
             }
             cp_async_commit();
         }
-        cp_async_wait<1>();    // everything but the prefetch just issued has landed
+#ifdef FBP_TRACE
+        if (it == 0) { cp_async_wait<3>(); __syncthreads(); FBP_TRACE_MARK(5); }
+#endif
+        if (it == 0) cp_async_wait<2>();   // taps and row 0 (rho and the prefetch may still be in flight)
+        else cp_async_wait<1>();           // everything but the prefetch just issued has landed
         __syncthreads();
+        FBP_TRACE_MARK(1);
 
         // ---- compute: R output pairs x this warp's slice of the inputs (chunks of 2R inputs) ----
         {
@@ -222,7 +243,9 @@ filter2_kernel(const T* __restrict__ P, T* __restrict__ Q, uint4* __restrict__ E
 #pragma unroll
             for (int r = 0; r < R; ++r) { pp[2 * r] = acc[r].hi(); pp[2 * r + 1] = acc[r].lo(); }
         }
+        if (it == 0) cp_async_wait<1>();   // rho
         __syncthreads();
+        FBP_TRACE_MARK(2);
 
         // ---- fixed-order reduction over input slices, centre tap, conditioning term, scale ----
         // yz[k] = Q~[k - 1 - guard]: the row in natural order with zero guards (store_entries)
@@ -239,6 +262,7 @@ filter2_kernel(const T* __restrict__ P, T* __restrict__ Q, uint4* __restrict__ E
             yz[k] = y;
         }
         __syncthreads();
+        FBP_TRACE_MARK(3);
 
         // ---- stores: plain row and/or interleaved entries, coalesced ----
         if (Q) {
@@ -250,6 +274,8 @@ filter2_kernel(const T* __restrict__ P, T* __restrict__ Q, uint4* __restrict__ E
                                 wrow ? wrow + row % n_angles : nullptr);
     }
     cp_async_wait<0>();
+    __syncthreads();
+    FBP_TRACE_MARK(4);
 }
 
 }  // namespace fbp
