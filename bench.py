@@ -338,7 +338,7 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the back-projection kernel, per launch, from
 # the committed `ncu --set full` capture (profiles/); None until a capture for that key exists.
-NCU_TRAFFIC_BYTES = {(3, "f32"): 2967808}   # profiles/r1b_bp_cfg3_f32_ncu_full.txt (ncu flushes caches per replay pass)
+NCU_TRAFFIC_BYTES = {(3, "f32"): 2968320}   # profiles/r1d_bp_cfg3_f32_ncu_full.txt (ncu flushes caches per replay pass)
 
 
 def main():
