@@ -94,11 +94,12 @@ fbp_status fbp_reconstruct(fbp_plan *plan, const void *d_sino, void *d_image, in
                            void *cuda_stream);
 
 /*
- * fbp_reconstruct_host -- the same reconstruction for HOST buffers: copies h_sino
- * [batch][K][D] to a plan-owned device buffer, runs fbp_reconstruct, copies the image
- * back to h_image [batch][N][N], and waits for the stream.  Pinned host memory makes the
- * copies asynchronous until the final wait; pageable memory works too.  This is the
- * end-to-end path bench.py's "e2e" leg times (copies inside the timed region).
+ * fbp_reconstruct_host -- the same reconstruction for HOST buffers: h_sino [batch][K][D] in, h_image
+ * [batch][N][N] out, then waits for the stream.  This is the end-to-end path bench.py's "e2e" leg times
+ * (transfers inside the timed region).  The sinogram is copied to a plan-owned device buffer (for stacks
+ * of >= 8 slices group by group, overlapping the previous group's back-projection).  If h_image is pinned
+ * (page-locked, device-accessible) memory the back-projector stores its pixels straight into it over PCIe,
+ * overlapped with the kernel; pageable memory takes a device image and a copy.  Same bytes either way.
  */
 fbp_status fbp_reconstruct_host(fbp_plan *plan, const void *h_sino, void *h_image, int batch,
                                 void *cuda_stream);

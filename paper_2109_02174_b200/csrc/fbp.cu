@@ -84,6 +84,7 @@ struct fbp_plan {
 
     double* d_mscratch = nullptr;   // fbp_metrics: [kMetricGrid][3] CTA partials, then mid[3]
     bool use_pdl = true;
+    bool host_zero_copy = true;   // fbp_reconstruct_host: store results straight into pinned host memory
     // batch pipeline (run_pipelined): filter of slice group g+1 overlaps back-projection of group g
     static constexpr int kMaxGroups = 16;
     int pipe_min_batch = 8, pipe_group = 0;
@@ -588,7 +589,8 @@ fbp_status run_bp(fbp_plan* p, const void* filt, void* image, int batch, cudaStr
 // plan-owned streams (two, so that the tail of one launch overlaps the head of the next).  The
 // caller's stream forks into them and joins at the end: still enqueue-only, no host wait.  Same
 // kernels on the same data as the sequential path, hence the same bytes.
-fbp_status run_pipelined(fbp_plan* p, const void* sino, void* image, int batch, cudaStream_t s)
+fbp_status run_pipelined(fbp_plan* p, const void* sino, void* image, int batch, cudaStream_t s,
+                         const void* h_sino = nullptr)
 {
     int group = p->pipe_group > 0 ? p->pipe_group : (batch + 3) / 4;   // 4 groups measured best at 64 slices
     const int min_group = (batch + fbp_plan::kMaxGroups - 1) / fbp_plan::kMaxGroups;
@@ -604,6 +606,11 @@ fbp_status run_pipelined(fbp_plan* p, const void* sino, void* image, int batch, 
         const int g0 = g * group, nb = batch - g0 < group ? batch - g0 : group;
         const char* sg = static_cast<const char*>(sino) + (size_t)g0 * sino_slice;
         char* eg = static_cast<char*>(p->d_ent) + (size_t)g0 * ent_slice;
+        // host source (fbp_reconstruct_host): this group's copy rides the filter stream, so it overlaps the
+        // back-projection of the previous group on the copy engine
+        if (h_sino)
+            FBP_CUDA(p, cudaMemcpyAsync(const_cast<char*>(sg), static_cast<const char*>(h_sino) + (size_t)g0 * sino_slice,
+                                        (size_t)nb * sino_slice, cudaMemcpyHostToDevice, p->st_f));
         cudaError_t e = p->dtype == FBP_F32 ? launch_filter2<float>(p, sg, nullptr, eg, nb, p->st_f)
                                             : launch_filter2<double>(p, sg, nullptr, eg, nb, p->st_f);
         if (e != cudaSuccess) return cuda_fail(p, e, "filter launch");
@@ -683,6 +690,7 @@ fbp_status fbp_create(fbp_plan** out, int n_angles, int n_det, const double* ang
     configure_filter2_dense(p);
     p->filter_v = env_int("FBP_FILTER_V", 2) == 1 ? 1 : 2;
     p->use_pdl = env_int("FBP_PDL", 1) != 0;
+    p->host_zero_copy = env_int("FBP_HOST_ZERO_COPY", 1) != 0;
 
     auto bail = [&](fbp_status st) { std::string m = p->err; fbp_destroy(p); g_create_error = m; return st; };
     if (p->filter_v == 2 && (p->f2_threads > 512 || p->f2_smem > 220 * 1024)) p->filter_v = 1;
@@ -896,19 +904,34 @@ fbp_status fbp_reconstruct_host(fbp_plan* p, const void* h_sino, void* h_image, 
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const size_t sino_bytes = p->esize * (size_t)p->K * p->D, img_bytes = p->esize * (size_t)p->N * p->N;
     if (!p->d_hsino) FBP_CUDA(p, cudaMalloc(&p->d_hsino, sino_bytes * p->max_batch));
-    if (!p->d_himg) FBP_CUDA(p, cudaMalloc(&p->d_himg, img_bytes * p->max_batch));
-    FBP_CUDA(p, cudaMemcpyAsync(p->d_hsino, h_sino, sino_bytes * batch, cudaMemcpyHostToDevice, s));
+    // Result: if h_image is pinned (device-accessible) host memory, the back-projector stores its pixels straight
+    // into it -- coalesced 128-byte posted writes over PCIe that overlap the kernel -- instead of a device image
+    // followed by a copy.  Pageable memory takes the staged path.
+    void* img_target = nullptr;
+    {
+        cudaPointerAttributes attr{};
+        if (cudaPointerGetAttributes(&attr, h_image) == cudaSuccess && attr.type == cudaMemoryTypeHost &&
+            attr.devicePointer != nullptr && aligned16(attr.devicePointer) && p->host_zero_copy)
+            img_target = attr.devicePointer;
+        cudaGetLastError();
+    }
+    const bool staged = img_target == nullptr;
+    if (staged) {
+        if (!p->d_himg) FBP_CUDA(p, cudaMalloc(&p->d_himg, img_bytes * p->max_batch));
+        img_target = p->d_himg;
+    }
     p->ran_filter = p->ran_bp = false;
     fbp_status st;
     if (use_pipeline(p, batch)) {
-        st = run_pipelined(p, p->d_hsino, p->d_himg, batch, s);
+        st = run_pipelined(p, p->d_hsino, img_target, batch, s, h_sino);
     } else {
+        FBP_CUDA(p, cudaMemcpyAsync(p->d_hsino, h_sino, sino_bytes * batch, cudaMemcpyHostToDevice, s));
         st = run_filter(p, p->d_hsino, nullptr, p->d_ent, batch, s);
         if (st != FBP_OK) return st;
-        st = run_bp(p, nullptr, p->d_himg, batch, s);
+        st = run_bp(p, nullptr, img_target, batch, s);
     }
     if (st != FBP_OK) return st;
-    FBP_CUDA(p, cudaMemcpyAsync(h_image, p->d_himg, img_bytes * batch, cudaMemcpyDeviceToHost, s));
+    if (staged) FBP_CUDA(p, cudaMemcpyAsync(h_image, p->d_himg, img_bytes * batch, cudaMemcpyDeviceToHost, s));
     FBP_CUDA(p, cudaStreamSynchronize(s));
     return FBP_OK;
 }

@@ -342,3 +342,25 @@ def test_long_rows_and_many_angles(fbp, oracle):
         check_image(f, oracle.reconstruct(sino, ang, n), "f64", "many angles")
     finally:
         plan.close()
+
+
+@pytest.mark.parametrize("batch", [1, 11])
+@pytest.mark.parametrize("pinned", [True, False])
+def test_host_path_pinned_pageable_and_batched(fbp, pinned, batch):
+    """fbp_reconstruct_host: pinned results are written by the kernel straight into host memory, pageable ones are
+    staged and copied; stacks go through the batch pipeline with per-group copies.  All must equal the device path."""
+    torch = _torch()
+    n, k, dd = 80, 40, 115
+    sino = torch.from_numpy(I.random_sinogram(8, batch, k, dd).astype(np.float32))
+    host = torch.full((batch, n, n), 7.0, dtype=torch.float32)
+    if pinned:
+        sino, host = sino.pin_memory(), host.pin_memory()
+    plan = fbp.Plan(list(I.uniform_angles(k)), dd, n, dtype="f32", max_batch=batch)
+    try:
+        dev = plan.reconstruct(sino.cuda())
+        for _ in range(2):
+            fbp.fbp_reconstruct_host(plan.handle, sino, host, batch)
+            assert torch.equal(dev.cpu(), host)
+            host.fill_(7.0)
+    finally:
+        plan.close()
