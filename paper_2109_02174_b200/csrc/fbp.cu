@@ -925,8 +925,22 @@ fbp_status fbp_reconstruct_host(fbp_plan* p, const void* h_sino, void* h_image, 
     if (use_pipeline(p, batch)) {
         st = run_pipelined(p, p->d_hsino, img_target, batch, s, h_sino);
     } else {
-        FBP_CUDA(p, cudaMemcpyAsync(p->d_hsino, h_sino, sino_bytes * batch, cudaMemcpyHostToDevice, s));
-        st = run_filter(p, p->d_hsino, nullptr, p->d_ent, batch, s);
+        // Small pinned sinograms are read by the filter straight from host memory (each row once, by cp.async):
+        // the rows stream in over PCIe while earlier rows are already being filtered, and one copy operation with
+        // its launch gap disappears.  Large or pageable ones are copied first.
+        const void* sino_src = p->d_hsino;
+        {
+            cudaPointerAttributes attr{};
+            const int in_mode = env_int("FBP_HOST_ZERO_COPY_IN", 1);
+            if (in_mode && p->host_zero_copy && sino_bytes * batch <= ((size_t)8 << 20) &&
+                cudaPointerGetAttributes(&attr, h_sino) == cudaSuccess && attr.type == cudaMemoryTypeHost &&
+                attr.devicePointer != nullptr && aligned16(attr.devicePointer))
+                sino_src = attr.devicePointer;
+            cudaGetLastError();
+        }
+        if (sino_src == p->d_hsino)
+            FBP_CUDA(p, cudaMemcpyAsync(p->d_hsino, h_sino, sino_bytes * batch, cudaMemcpyHostToDevice, s));
+        st = run_filter(p, sino_src, nullptr, p->d_ent, batch, s);
         if (st != FBP_OK) return st;
         st = run_bp(p, nullptr, img_target, batch, s);
     }
