@@ -132,6 +132,24 @@ struct DeviceGuard {
 
 int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
+// The dynamic shared-memory limit is an attribute of the KERNEL (per context), not of a plan: plans with
+// different geometries share the instantiations, so each one is opened up once to the device maximum
+// (227 KB on sm_100, less the kernel's static shared memory) instead of to whatever the first plan needed.
+constexpr int kMaxDynSmem = 227 * 1024;
+constexpr int kMaxDevices = 64;
+template <typename Kern>
+cudaError_t allow_max_smem(Kern kern, bool (&done)[kMaxDevices], int device)
+{
+    const bool tracked = device >= 0 && device < kMaxDevices;
+    if (tracked && done[device]) return cudaSuccess;
+    cudaFuncAttributes fa{};
+    cudaError_t e = cudaFuncGetAttributes(&fa, kern);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem - (int)fa.sharedSizeBytes);
+    if (e == cudaSuccess && tracked) done[device] = true;
+    return e;
+}
+
 // ---- filter launch configuration -------------------------------------------------
 // One CTA per row; warps = 2 parities x n_ob output blocks (32*R outputs) x n_sb input slices.
 void configure_filter(fbp_plan* p)
@@ -443,11 +461,11 @@ cudaError_t launch_filter2_r(fbp_plan* p, const void* sino, void* filt, void* en
     const int threads = DENSE ? p->f2d_threads : p->f2_threads, smem = DENSE ? p->f2d_smem : p->f2_smem;
     int& cap = DENSE ? p->f2d_grid_cap : p->f2_grid_cap;
     auto kern = fbp::filter2_kernel<T, R, DENSE>;
+    static bool smem_open[kMaxDevices] = {};
+    if (cudaError_t e = allow_max_smem(kern, smem_open, p->device); e != cudaSuccess) return e;
     if (cap == 0) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
         int per_sm = 0;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem);
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem);
         if (e != cudaSuccess) return e;
         if (per_sm < 1) return cudaErrorLaunchOutOfResources;
         cap = per_sm * kNumSm;
@@ -483,23 +501,23 @@ cudaError_t launch_filter2(fbp_plan* p, const void* sino, void* filt, void* ent,
 }
 
 template <typename T>
-cudaError_t launch_entries(const fbp_plan* p, const void* filt, int batch, cudaStream_t st)
+cudaError_t launch_entries(fbp_plan* p, const void* filt, int batch, cudaStream_t st)
 {
     const size_t smem = (size_t)(p->bp.ent_pitch + 2) * sizeof(T);
     auto kern = fbp::entries_kernel<T>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
+    static bool smem_open[kMaxDevices] = {};
+    if (cudaError_t e = allow_max_smem(kern, smem_open, p->device); e != cudaSuccess) return e;
     kern<<<batch * p->K, 256, smem, st>>>(static_cast<const T*>(filt), static_cast<uint4*>(p->d_ent), p->D,
                                           p->bp.ent_pitch, p->bp.ent_guard, static_cast<const T*>(p->d_wrow), p->K);
     return cudaGetLastError();
 }
 
 template <typename T, int R, int WY, int WA>
-cudaError_t launch_bp_v(const fbp_plan* p, void* image, int batch, cudaStream_t st, int slice0)
+cudaError_t launch_bp_v(fbp_plan* p, void* image, int batch, cudaStream_t st, int slice0)
 {
     auto kern = fbp::backproject_kernel<T, R, WY, WA>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, p->bp_smem);
-    if (e != cudaSuccess) return e;
+    static bool smem_open[kMaxDevices] = {};     // per instantiation and device
+    if (cudaError_t e = allow_max_smem(kern, smem_open, p->device); e != cudaSuccess) return e;
     // programmatic dependent launch: the CTAs may become resident and run their prologue while the
     // kernel that writes the entries (filter / entries_kernel) drains; the producer warp executes
     // griddepcontrol.wait before its first read of the entries
@@ -522,7 +540,7 @@ cudaError_t launch_bp_v(const fbp_plan* p, void* image, int batch, cudaStream_t 
 
 // back-projection of the plan's entry buffer into `image`
 template <typename T>
-cudaError_t launch_bp(const fbp_plan* p, void* image, int batch, cudaStream_t st, int slice0 = 0)
+cudaError_t launch_bp(fbp_plan* p, void* image, int batch, cudaStream_t st, int slice0 = 0)
 {
     switch (p->bp_variant) {
         case 0: return launch_bp_v<T, 8, 4, 1>(p, image, batch, st, slice0);
