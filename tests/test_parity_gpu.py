@@ -364,3 +364,28 @@ def test_host_path_pinned_pageable_and_batched(fbp, pinned, batch):
             host.fill_(7.0)
     finally:
         plan.close()
+
+
+def test_plans_of_different_geometry_interleaved(fbp, oracle):
+    """Kernel attributes (dynamic shared-memory limits) belong to the kernel, not to a plan: plans with small and
+    large rows/tiles, created first and used later in any order, must all keep working and stay independent."""
+    torch = _torch()
+    big = fbp.Plan(list(I.config_angles(3)), 725, 512, dtype="f32")
+    small = fbp.Plan(list(I.uniform_angles(6)), 24, 16, dtype="f32")
+    mid = fbp.Plan(list(I.uniform_angles(50)), 2001, 64, dtype="f32")
+    try:
+        s_small = I.random_sinogram(1, 1, 6, 24).astype(np.float32)
+        s_mid = I.random_sinogram(2, 1, 50, 2001).astype(np.float32)
+        s_big = I.config_sinogram(3).astype(np.float32)
+        outs = {}
+        for name in ("small", "big", "mid", "small", "big", "mid"):
+            plan, sino = {"small": (small, s_small), "big": (big, s_big), "mid": (mid, s_mid)}[name]
+            out = plan.reconstruct(_to_dev(sino, "f32"))
+            torch.cuda.synchronize()
+            if name in outs:
+                assert torch.equal(out, outs[name])
+            outs[name] = out.clone()
+        check_image(outs["small"].cpu().numpy(), oracle.reconstruct(s_small.astype(np.float64), I.uniform_angles(6), 16), "f32", "small")
+        check_image(outs["mid"].cpu().numpy(), oracle.reconstruct(s_mid.astype(np.float64), I.uniform_angles(50), 64), "f32", "mid")
+    finally:
+        big.close(); small.close(); mid.close()
