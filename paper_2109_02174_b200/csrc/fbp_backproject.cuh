@@ -171,8 +171,14 @@ template <> struct PairAcc<double> {
 // cs2: [K] pairs (cos*pix/d, sin*pix/d) in fp64.  E: 16-byte entry units [batch][K][planes][pitch].
 // Grid (tiles, S, batch).  image: [batch][N][N], fully written, scaled by pi/K.
 // part: scratch [S][batch][N][N] and tickets: [batch][tiles] zero-initialised counters (S > 1 only).
+// Registers per thread the occupancy bound aims at.  fp32: 64 for the small-tile variants (6 CTAs of 160 threads per SM),
+// 72 for the 32x32 tile (R = 8, WY = 4: at 64 the 16 packed accumulators spill 48 bytes; measured 1.84 -> 1.78 ms at
+// config 5, 2.88 -> 2.84 ms at config 4).  fp64: 96, and 112 for the 32x32 tile (3.60 -> 3.52 ms at config 5).
+#ifndef FBP_BP_REGCAP64
+#define FBP_BP_REGCAP64 ((R == 8 && WY == 4 && WA == 1) ? 112 : 96)
+#endif
 #ifndef FBP_BP_REGCAP
-#define FBP_BP_REGCAP (sizeof(T) == 4 ? 64 : 96)
+#define FBP_BP_REGCAP (sizeof(T) == 4 ? ((R == 8 && WY == 4 && WA == 1) ? 72 : 64) : FBP_BP_REGCAP64)
 #endif
 #ifndef FBP_BP_STAGES
 #define FBP_BP_STAGES 3
