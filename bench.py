@@ -235,6 +235,7 @@ def run_ours(args):
     # slice (r*B + s) of the recipe, so ranks do not share inputs.  Big stacks reuse 4 distinct slices.
     distinct = min(B, 4)
     base = np.stack([I.config_slice(args.config, rank * B + s) for s in range(distinct)]).astype(npdt)
+    input_sha = I.sha256(base)                       # ties the result to the bytes that were reconstructed
     h_sino = torch.from_numpy(base[np.arange(B) % distinct].copy()).pin_memory()
     d_sino = h_sino.cuda()
     d_img = torch.empty((B, N, N), dtype=tdt, device="cuda")
@@ -333,7 +334,7 @@ def run_ours(args):
     return dict(world=world, rank=rank, cfg=cfg, info=info, ms_step=ms_step, f_ms=f_ms, b_ms=b_ms, e2e_s=e2e_s,
                 updates=updates, clocks=clk.summary(), esize=h_sino.element_size(),
                 h2d=h_sino.numel() * h_sino.element_size(), d2h=h_img.numel() * h_img.element_size(), plan=plan,
-                extras=extras)
+                extras=extras, input_sha=input_sha)
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the back-projection kernel, per launch, from
@@ -392,6 +393,7 @@ def main():
         "clocks": r["clocks"],
     }
     line["config"]["window"] = args.window
+    line["config"]["input_sha256"] = r["input_sha"]
     if r["extras"]:
         line["extras"] = dict(r["extras"], metrics_hbm_frac=r["extras"]["metrics_gbs"] / float(peaks["hbm_gbs"]),
                               stack_interp_hbm_frac=r["extras"]["stack_interp_gbs"] / float(peaks["hbm_gbs"]))
