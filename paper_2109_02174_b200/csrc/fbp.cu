@@ -839,6 +839,7 @@ fbp_status fbp_create(fbp_plan** out, int n_angles, int n_det, const double* ang
         FBP_TRY(cudaMemset(p->d_tickets, 0, sizeof(int) * nt));
     }
     FBP_TRY(cudaMalloc(&p->d_mscratch, sizeof(double) * (3 * kMetricGrid + 4)));
+    FBP_TRY(cudaMemset(p->d_mscratch, 0, sizeof(double) * (3 * kMetricGrid + 4)));
     for (int i = 0; i < 4; ++i) FBP_TRY(cudaEventCreate(&p->ev[i]));
     p->pipe_min_batch = env_int("FBP_PIPE_MIN_BATCH", 8);
     p->pipe_group = env_int("FBP_PIPE_GROUP", 0);
@@ -976,14 +977,14 @@ static cudaError_t launch_metrics(fbp_plan* p, const void* x, const void* y, lon
 {
     double* partial = p->d_mscratch;
     double* mid = p->d_mscratch + 3 * kMetricGrid;
-    long long want = (n + fbp::kMetricThreads - 1) / fbp::kMetricThreads;
+    // at least 32 elements per thread: small inputs get few CTAs (fewer partials, fewer tickets on one counter)
+    long long want = (n + 32LL * fbp::kMetricThreads - 1) / (32LL * fbp::kMetricThreads);
     const int grid = (int)(want < kMetricGrid ? (want < 1 ? 1 : want) : kMetricGrid);
     const T* a = static_cast<const T*>(x);
     const T* b = static_cast<const T*>(y);
-    fbp::metrics_partial_kernel<T, 0><<<grid, fbp::kMetricThreads, 0, st>>>(a, b, n, mid, partial);
-    fbp::metrics_final_kernel<0><<<1, 32, 0, st>>>(partial, grid, n, mid, max_val, c1, c2, d_out);
-    fbp::metrics_partial_kernel<T, 1><<<grid, fbp::kMetricThreads, 0, st>>>(a, b, n, mid, partial);
-    fbp::metrics_final_kernel<1><<<1, 32, 0, st>>>(partial, grid, n, mid, max_val, c1, c2, d_out);
+    unsigned* ticket = reinterpret_cast<unsigned*>(mid + 3);      // zero-initialised at fbp_create, self re-arming
+    fbp::metrics_partial_kernel<T, 0><<<grid, fbp::kMetricThreads, 0, st>>>(a, b, n, mid, partial, ticket, max_val, c1, c2, d_out);
+    fbp::metrics_partial_kernel<T, 1><<<grid, fbp::kMetricThreads, 0, st>>>(a, b, n, mid, partial, ticket, max_val, c1, c2, d_out);
     return cudaGetLastError();
 }
 

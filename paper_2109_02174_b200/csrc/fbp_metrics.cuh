@@ -5,7 +5,7 @@
 //   SSIM = (2 mu_x mu_y + C1)(2 s_xy + C2) / ((mu_x^2 + mu_y^2 + C1)(s_x^2 + s_y^2 + C2)),
 //   mu = mean, s^2 / s_xy = population (co)variances over the whole image (the paper gives no window).
 //
-// Two passes, like the definition: pass 0 sums x, y, (x-y)^2; a one-CTA step turns them into the
+// Two passes (two launches), like the definition: pass 0 sums x, y, (x-y)^2 and its last CTA turns them into the
 // means; pass 1 sums the centred products (x-mu_x)^2, (y-mu_y)^2, (x-mu_x)(y-mu_y).  All sums are
 // fp64 whatever the image dtype.  Determinism: a fixed grid, every thread walks a fixed strided
 // index set, lanes are combined with a fixed shuffle tree, warps and CTAs in index order -- no
@@ -19,11 +19,42 @@ namespace fbp {
 
 constexpr int kMetricThreads = 256;
 
+// Run by the first warp of the last CTA: CTA partials are added in index order by lane-strided sums + the shuffle tree.
+// PASS 0: mid[0..2] = (mu_x, mu_y, MSE).   PASS 1: out[0..7] = MSE, PSNR, SSIM, mu_x, mu_y, s_x^2, s_y^2, s_xy.
+template <int PASS>
+__device__ __forceinline__ void metrics_finish(const double* partial, int n_partial, long long n, double* mid,
+                                               double max_val, double c1, double c2, double* out)
+{
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+    for (int i = threadIdx.x; i < n_partial; i += 32) {
+        s0 += __ldcg(partial + 3 * i + 0); s1 += __ldcg(partial + 3 * i + 1); s2 += __ldcg(partial + 3 * i + 2);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        s0 += __shfl_down_sync(0xffffffffu, s0, o);
+        s1 += __shfl_down_sync(0xffffffffu, s1, o);
+        s2 += __shfl_down_sync(0xffffffffu, s2, o);
+    }
+    if (threadIdx.x != 0) return;
+    const double inv_n = 1.0 / (double)n;
+    if (PASS == 0) {
+        mid[0] = s0 * inv_n; mid[1] = s1 * inv_n; mid[2] = s2 * inv_n;
+    } else {
+        const double mx = mid[0], my = mid[1], mse = mid[2];
+        const double vx = s0 * inv_n, vy = s1 * inv_n, cxy = s2 * inv_n;
+        out[0] = mse;
+        out[1] = mse > 0.0 ? 20.0 * log10(max_val / sqrt(mse)) : __longlong_as_double(0x7ff0000000000000ll);
+        out[2] = ((2.0 * mx * my + c1) * (2.0 * cxy + c2)) / ((mx * mx + my * my + c1) * (vx + vy + c2));
+        out[3] = mx; out[4] = my; out[5] = vx; out[6] = vy; out[7] = cxy;
+    }
+}
+
 // partial: [gridDim.x][3] doubles.  PASS 0: (sum x, sum y, sum (x-y)^2);  PASS 1: centred, means from `mid`.
 template <typename T, int PASS>
 __global__ void __launch_bounds__(kMetricThreads)
 metrics_partial_kernel(const T* __restrict__ x, const T* __restrict__ y, long long n,
-                       const double* __restrict__ mid, double* __restrict__ partial)
+                       double* __restrict__ mid, double* __restrict__ partial, unsigned* __restrict__ ticket,
+                       double max_val, double c1, double c2, double* __restrict__ out)
 {
     double mx = 0.0, my = 0.0;
     if (PASS == 1) { mx = mid[0]; my = mid[1]; }
@@ -83,37 +114,19 @@ metrics_partial_kernel(const T* __restrict__ x, const T* __restrict__ y, long lo
         partial[3 * blockIdx.x + 1] = t1;
         partial[3 * blockIdx.x + 2] = t2;
     }
-}
-
-// One CTA of 32 threads; CTA partials are added in index order by lane-strided sums + the shuffle tree.
-// PASS 0: mid[0..2] = (mu_x, mu_y, MSE).   PASS 1: out[0..7] = MSE, PSNR, SSIM, mu_x, mu_y, s_x^2, s_y^2, s_xy.
-template <int PASS>
-__global__ void __launch_bounds__(32)
-metrics_final_kernel(const double* __restrict__ partial, int n_partial, long long n, double* __restrict__ mid,
-                     double max_val, double c1, double c2, double* __restrict__ out)
-{
-    double s0 = 0.0, s1 = 0.0, s2 = 0.0;
-    for (int i = threadIdx.x; i < n_partial; i += 32) {
-        s0 += partial[3 * i + 0]; s1 += partial[3 * i + 1]; s2 += partial[3 * i + 2];
+    // The CTA that draws the last ticket (ordering only, never data) adds the CTA partials in index order --
+    // the same order whichever CTA that is -- and finishes the pass: means (pass 0) or the eight outputs (pass 1).
+    __shared__ bool s_last;
+    if (threadIdx.x == 0) {
+        __threadfence();
+        const unsigned t = atomicAdd(ticket, 1u);
+        s_last = (t == gridDim.x - 1);
+        if (s_last) *ticket = 0u;                 // re-arm for the next pass / call
     }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        s0 += __shfl_down_sync(0xffffffffu, s0, o);
-        s1 += __shfl_down_sync(0xffffffffu, s1, o);
-        s2 += __shfl_down_sync(0xffffffffu, s2, o);
-    }
-    if (threadIdx.x != 0) return;
-    const double inv_n = 1.0 / (double)n;
-    if (PASS == 0) {
-        mid[0] = s0 * inv_n; mid[1] = s1 * inv_n; mid[2] = s2 * inv_n;
-    } else {
-        const double mx = mid[0], my = mid[1], mse = mid[2];
-        const double vx = s0 * inv_n, vy = s1 * inv_n, cxy = s2 * inv_n;
-        out[0] = mse;
-        out[1] = mse > 0.0 ? 20.0 * log10(max_val / sqrt(mse)) : __longlong_as_double(0x7ff0000000000000ll);
-        out[2] = ((2.0 * mx * my + c1) * (2.0 * cxy + c2)) / ((mx * mx + my * my + c1) * (vx + vy + c2));
-        out[3] = mx; out[4] = my; out[5] = vx; out[6] = vy; out[7] = cxy;
-    }
+    __syncthreads();
+    if (!s_last || threadIdx.x >= 32) return;
+    __threadfence();
+    metrics_finish<PASS>(partial, (int)gridDim.x, n, mid, max_val, c1, c2, out);
 }
 
 }  // namespace fbp
