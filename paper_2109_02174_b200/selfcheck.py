@@ -54,5 +54,45 @@ def main() -> int:
     return 0
 
 
+def soak(runs: int) -> int:
+    """``--soak N``: N reconstructions per case with other work interleaved; every 25th result and the last are
+    compared bit for bit with the first (the paper's parallel versions differed on every run)."""
+    import numpy as np
+    import torch
+
+    import paper_2109_02174_b200 as pkg
+    from paper_2109_02174_b200 import inputs as I
+
+    pkg.load_library()
+    torch.cuda.set_device(0)
+    bad = 0
+    for cid, dt, batch, env in ((3, "f32", 1, {}), (3, "f64", 1, {}), (3, "f32", 1, {"FBP_BP_SPLITS": "3"}),
+                                (2, "f32", 12, {}), (1, "f32", 1, {})):
+        os.environ.update(env)
+        try:
+            cfg = I.CONFIGS[cid]
+            tdt = torch.float32 if dt == "f32" else torch.float64
+            sino = torch.from_numpy(np.stack([I.config_slice(cid, s % 3) for s in range(batch)])).to(tdt).cuda()
+            with pkg.Plan(list(I.config_angles(cid)), cfg.n_det, cfg.image_n, dtype=dt, max_batch=batch) as plan:
+                first = plan.reconstruct(sino).clone()
+                junk = torch.randn(2048, 2048, device="cuda")
+                miss = 0
+                for i in range(runs):
+                    if i % 7 == 0:
+                        junk = (junk @ junk) * 1e-4
+                    out = plan.reconstruct(sino)
+                    if i % 25 == 0 or i == runs - 1:
+                        miss += int(not torch.equal(out, first))
+                torch.cuda.synchronize()
+            print("cfg%d %s batch %d %s: %d runs, %d mismatches" % (cid, dt, batch, env, runs, miss))
+            bad += miss
+        finally:
+            for key in env:
+                os.environ.pop(key, None)
+    return 1 if bad else 0
+
+
 if __name__ == "__main__":
+    if len(sys.argv) > 2 and sys.argv[1] == "--soak":
+        sys.exit(soak(int(sys.argv[2])))
     sys.exit(main())
