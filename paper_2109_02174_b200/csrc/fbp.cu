@@ -1022,7 +1022,7 @@ fbp_status fbp_project(fbp_plan* p, const void* d_image, void* d_sino, int batch
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     fbp::ProjParams prm{p->K, p->D, p->N, pad, 0.5 * (p->N - 1), 0.5 * (p->D - 1)};
     const dim3 tgrid((p->N + 31) / 32, (p->N + 31) / 32, batch), tblock(32, 8);
-    const dim3 pgrid((p->D + 127) / 128, p->K, batch);
+    const dim3 pgrid(((p->D + 1) / 2 + 127) / 128, p->K, batch);     // a thread owns a bin and its mirror bin
     if (p->dtype == FBP_F32) {
         float* xp = static_cast<float*>(p->d_xt);
         float* xtp = xp + (size_t)p->max_batch * plane;

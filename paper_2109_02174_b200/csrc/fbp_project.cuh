@@ -70,7 +70,10 @@ stage_image_kernel(const T* __restrict__ x, T* __restrict__ xp, T* __restrict__ 
         }
 }
 
-// cs2: [K] (cos, sin) * pix/d in fp64.  Grid (ceil(D/128), K, batch), block 128: thread = bin j.
+// Point symmetry (as in the back-projector): the mirror pixel (N-1-l, N-1-p) has u' = (D-1) - u, so it meets the
+// mirror bin D-1-j with the SAME weight hat(u - j).  A thread therefore owns bin j < ceil(D/2) and its mirror bin
+// and computes the run and its weights once for both.
+// cs2: [K] (cos, sin) * pix/d in fp64.  Grid (ceil(ceil(D/2)/128), K, batch), block 128: thread = bin j.
 // xp / xtp: the padded image and its padded transpose (stage_image_kernel).  y: [batch][K][D], fully written.
 template <typename T>
 __global__ void __launch_bounds__(128)
@@ -80,7 +83,8 @@ project_kernel(const T* __restrict__ xp, const T* __restrict__ xtp, T* __restric
     const int j = blockIdx.x * 128 + threadIdx.x;
     const int i = blockIdx.y, b = blockIdx.z;
     const int N = prm.image_n, pitch = N + 2 * prm.pad;
-    if (j >= prm.n_det) return;
+    if (j >= (prm.n_det + 1) / 2) return;
+    const int jm = prm.n_det - 1 - j;            // mirror bin (== j for the middle bin of an odd detector)
     const double2 cs = cs2[i];
     const bool xmajor = fabs(cs.x) >= fabs(cs.y);
     const double cf = xmajor ? cs.x : cs.y;      // change of u per pixel along a line (fast axis); |cf| > 0
@@ -106,7 +110,8 @@ project_kernel(const T* __restrict__ xp, const T* __restrict__ xtp, T* __restric
     }
     const T BlT = (T)Bl;
     const int cmin = -(E + 1), cmax = N + E;     // clamp of round(p*): the run stays inside the zero pads
-    T acc = T(0);
+    T acc = T(0), accm = T(0);
+    const T* imgm = img + (size_t)(N - 1) * pitch + (N - 1);       // mirror of (line 0, pixel 0)
     // Lines in blocks of 32: p*(l0) in fp64 once per block, split into an integer part and a fraction; inside
     // the block the fraction advances in the working precision (|.| < 34: ulp <= 4e-6 in fp32) and is rounded
     // with the add-magic-constant trick.  No bounds checks: out-of-image pixels of a run read the zero pads.
@@ -117,6 +122,7 @@ project_kernel(const T* __restrict__ xp, const T* __restrict__ xtp, T* __restric
         const T fb = (T)(base - bfl);
         const int l1 = min(32, l_hi - l0 + 1);
         const T* line = img + (size_t)l0 * pitch;
+        const T* linem = imgm - (size_t)l0 * pitch;
         if (E == 1) {
 #pragma unroll 4
             for (int q = 0; q < l1; ++q) {
@@ -125,11 +131,14 @@ project_kernel(const T* __restrict__ xp, const T* __restrict__ xtp, T* __restric
                 const int p0 = min(max(pb + (int)(Magic<T>::bits(tm) - Magic<T>::kBits), cmin), cmax);   // round(p*)
                 const T d0 = ps - (tm - Magic<T>::m());                             // p* - round(p*), in [-1/2, 1/2]
                 const T* c = line + (size_t)q * pitch + p0;
+                const T* cm = linem - (size_t)q * pitch - p0;                       // mirror pixel of (line, p0)
                 const T vm = __ldg(c - 1), v0 = __ldg(c), vp = __ldg(c + 1);
+                const T um = __ldg(cm + 1), u0 = __ldg(cm), up = __ldg(cm - 1);
                 const T wm = fmax(fma(-acf, T(1) + d0, T(1)), T(0));                // e = -1: |e - d0| = 1 + d0
                 const T w0 = fmax(fma(-acf, fabs(d0), T(1)), T(0));
                 const T wp = fmax(fma(-acf, T(1) - d0, T(1)), T(0));
                 acc = fma(wm, vm, acc); acc = fma(w0, v0, acc); acc = fma(wp, vp, acc);
+                accm = fma(wm, um, accm); accm = fma(w0, u0, accm); accm = fma(wp, up, accm);
             }
         } else {
             for (int q = 0; q < l1; ++q) {
@@ -138,12 +147,18 @@ project_kernel(const T* __restrict__ xp, const T* __restrict__ xtp, T* __restric
                 const int p0 = min(max(pb + (int)(Magic<T>::bits(tm) - Magic<T>::kBits), cmin), cmax);
                 const T d0 = ps - (tm - Magic<T>::m());
                 const T* c = line + (size_t)q * pitch + p0;
-                for (int e = -E; e <= E; ++e)
-                    acc = fma(fmax(fma(-acf, fabs((T)e - d0), T(1)), T(0)), __ldg(c + e), acc);   // hat(u - j) x
+                const T* cm = linem - (size_t)q * pitch - p0;
+                for (int e = -E; e <= E; ++e) {
+                    const T w = fmax(fma(-acf, fabs((T)e - d0), T(1)), T(0));       // hat(u - j)
+                    acc = fma(w, __ldg(c + e), acc);
+                    accm = fma(w, __ldg(cm - e), accm);
+                }
             }
         }
     }
-    y[((size_t)b * prm.n_angles + i) * prm.n_det + j] = acc;
+    T* yrow = y + ((size_t)b * prm.n_angles + i) * prm.n_det;
+    yrow[j] = acc;
+    if (jm != j) yrow[jm] = accm;
 }
 
 }  // namespace fbp
