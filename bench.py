@@ -102,7 +102,7 @@ class ClockSampler:
                 self._once()
             except Exception:
                 pass
-            self._stop.wait(0.01)
+            self._stop.wait(0.002)
 
     def __enter__(self):
         if self.ok:
