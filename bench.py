@@ -339,7 +339,7 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the back-projection kernel, per launch, from
 # the committed `ncu --set full` capture (profiles/); None until a capture for that key exists.
-NCU_TRAFFIC_BYTES = {(3, "f32"): 2968320}   # profiles/r1d_bp_cfg3_f32_ncu_full.txt (ncu flushes caches per replay pass)
+NCU_TRAFFIC_BYTES = {(3, "f32"): 2968320, (3, "f64"): 5904640, (4, "f32"): 371400704 + 58770176}   # profiles/r1d_bp_cfg3_f32_ncu_full.txt, r1f_*.txt (ncu flushes caches per replay pass)
 
 
 def main():
