@@ -18,7 +18,11 @@
  *     against numerical quadrature of the defining integral (scipy), against the DTFT of the
  *     taps, and against the Ram-Lak taps of fbp_oracle.c for window 0.
  * W2  Per-angle weights (non-uniform angle sets): f = sum_i w_i q_i with
- *     caller-supplied w_i instead of pi/K each (eq. 2, weighted).
+ *     caller-supplied w_i instead of pi/K each (eq. 2, weighted).  Pinned in
+ *     tests/test_oracle_ext.py: uniform weights == the core back-projector; one-hot e_i == the core
+ *     back-projector on the sinogram with every row but i zeroed (x K/pi); random weights == the
+ *     dense brute-force matrix of P7 with the columns of angle i scaled by w_i (the last two fix
+ *     WHICH weight goes with WHICH angle).
  * M1  PSNR (eq. 3) and the global-statistics SSIM (eq. 4).
  */
 #include <math.h>

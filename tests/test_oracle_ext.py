@@ -79,6 +79,45 @@ def test_w2_weights_reduce_to_uniform_and_are_linear(oracle):
     assert np.allclose(one[5], 0.37 * np.interp(x, np.arange(d), q[0, 0]), rtol=1e-13)
 
 
+def test_w2_weight_i_belongs_to_angle_i(oracle):
+    """Pins the weight <-> angle ASSOCIATION (eq. 2 weighted) against code that is not the
+    weighted routine: (a) one-hot weight e_i == the core back-projector (pinned by P4-P7, P12) applied to the
+    sinogram with every row but i zeroed, times K/pi; (b) random non-uniform weights == the dense brute-force
+    matrix of P7 (independent triple loop, 8x8) with the columns of angle i scaled by w_i.
+    A mis-indexed weight (weights[K-1-i], weights[(i+1)%K]) fails both."""
+    n, k, d = 13, 7, 21
+    ang = np.sort(np.random.default_rng(31).uniform(0, PI, k))          # non-uniform: no angle symmetry to hide behind
+    q = I.random_sinogram(41, 1, k, d)[0]
+    for i in range(k):
+        only_i = np.zeros_like(q)
+        only_i[i] = q[i]
+        want = oracle.backproject(only_i, ang, n) * (k / PI)
+        got = oracle.backproject_weighted(q, ang, np.eye(k)[i], n)
+        assert np.allclose(got, want, rtol=1e-13, atol=1e-15), i
+        assert np.abs(want).max() > 0
+    # dense W (n^2 x K D) by an independent triple loop, columns of angle i scaled by w_i
+    n, k, d, dd, pix = 8, 5, 13, 1.0, 1.0
+    ang = np.sort(np.random.default_rng(32).uniform(0, PI, k))
+    w = np.random.default_rng(33).uniform(0.2, 2.0, k)
+    q = I.random_sinogram(42, 1, k, d)[0]
+    w_mat = np.zeros((n * n, k * d))
+    for r in range(n):
+        for c in range(n):
+            for i in range(k):
+                u = ((c - (n - 1) / 2) * pix * math.cos(ang[i]) + (r - (n - 1) / 2) * pix * math.sin(ang[i])) / dd + (d - 1) / 2
+                j = math.floor(u)
+                if 0 <= j < d:
+                    w_mat[r * n + c, i * d + j] += (1.0 - (u - j)) * w[i]
+                if 0 <= j + 1 < d:
+                    w_mat[r * n + c, i * d + j + 1] += (u - j) * w[i]
+    want = (w_mat @ q.ravel()).reshape(n, n)
+    assert np.allclose(oracle.backproject_weighted(q, ang, w, n), want, rtol=1e-13, atol=1e-14)
+    # and the batch axis keeps slices apart
+    q2 = I.random_sinogram(43, 2, k, d)
+    both = oracle.backproject_weighted(q2, ang, w, n)
+    assert np.allclose(both[1], (w_mat @ q2[1].ravel()).reshape(n, n), rtol=1e-13, atol=1e-14)
+
+
 def test_m1_psnr_ssim_closed_forms(oracle):
     rng = np.random.default_rng(8)
     x = rng.uniform(0, 1, (31, 29))
