@@ -44,6 +44,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--window", default="ramlak", choices=["ramlak", "shepp-logan", "cosine", "hamming", "hann"],
                     help="reconstruction filter (SURVEY.md 8(f) row 1); the headline is ramlak")
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=INT",
+                    help="launch-configuration override passed to fbp_create_tuned (A/B runs), e.g. --opt filter_sb=2")
     ap.add_argument("--extras", action="store_true", help="also time fbp_metrics (PSNR/SSIM) on the output stack")
     return ap.parse_args()
 
@@ -240,7 +242,8 @@ def run_ours(args):
     d_sino = h_sino.cuda()
     d_img = torch.empty((B, N, N), dtype=tdt, device="cuda")
     h_img = torch.empty((B, N, N), dtype=tdt).pin_memory()
-    plan = fbp.Plan(list(ang), D, N, dtype=args.dtype, max_batch=B)
+    options = {kv.split("=")[0]: int(kv.split("=")[1]) for kv in args.opt}
+    plan = fbp.Plan(list(ang), D, N, dtype=args.dtype, max_batch=B, options=options)
     if args.window != "ramlak":
         plan.set_window(args.window)
     info = plan.info()

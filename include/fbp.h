@@ -73,6 +73,41 @@ fbp_status fbp_create(fbp_plan **out, int n_angles, int n_det, const double *ang
                       int max_batch, int device);
 
 /*
+ * fbp_create_tuned -- fbp_create with explicit launch-configuration overrides, for tests, A/B measurements and
+ * bench.py.  h_options: HOST array of n_options (key, value) int pairs; keys not listed keep the library's
+ * choice; an unknown key is FBP_EINVAL.  The library never reads the environment: a plan's behaviour depends
+ * on these arguments only.  Options change launch shapes and summation grouping (hence possibly the last
+ * bits of a result), never the definition of what is computed; each plan stays bit-reproducible.
+ *   FBP_OPT_BP_VARIANT      index of the back-projection tile variant (R rows/thread, warps in y, angle groups)
+ *   FBP_OPT_BP_SPLITS       angle splits S per tile (>= 1)        FBP_OPT_BP_CHUNK   angles staged per chunk (<= 32)
+ *   FBP_OPT_FILTER_R        output pairs per thread of the direct-form filter (6, 10, 14; dense 5, 7, 9)
+ *   FBP_OPT_FILTER_SB       warps (input slices) per filter CTA (1..8)
+ *   FBP_OPT_FILTER_KIND     0 = library's choice, 1 = direct form, 2 = FFT form
+ *   FBP_OPT_PIPELINE        0 = no batch pipeline; FBP_OPT_PIPE_GROUP slices per pipeline group;
+ *   FBP_OPT_PIPE_MIN_BATCH  smallest batch that takes the pipeline (default 8)
+ *   FBP_OPT_PDL             0 = no programmatic dependent launch between filter and back-projector
+ *   FBP_OPT_HOST_ZERO_COPY  0 = fbp_reconstruct_host always stages through device buffers
+ *   FBP_OPT_BP_EVEN         0 = do not size shared memory for even CTA placement of small launches
+ */
+typedef enum {
+    FBP_OPT_BP_VARIANT = 1,
+    FBP_OPT_BP_SPLITS = 2,
+    FBP_OPT_BP_CHUNK = 3,
+    FBP_OPT_FILTER_R = 4,
+    FBP_OPT_FILTER_SB = 5,
+    FBP_OPT_FILTER_KIND = 6,
+    FBP_OPT_PIPELINE = 7,
+    FBP_OPT_PIPE_GROUP = 8,
+    FBP_OPT_PIPE_MIN_BATCH = 9,
+    FBP_OPT_PDL = 10,
+    FBP_OPT_HOST_ZERO_COPY = 11,
+    FBP_OPT_BP_EVEN = 13
+} fbp_option;
+fbp_status fbp_create_tuned(fbp_plan **out, int n_angles, int n_det, const double *angles_rad,
+                            double det_spacing, int image_n, double pixel_size, fbp_dtype dtype,
+                            int max_batch, int device, const int *h_options, int n_options);
+
+/*
  * fbp_filter -- Q = (1/d) h * P along the detector axis of every row.
  *   d_sino [batch][K][D] in, d_filtered [batch][K][D] out (may not alias).
  */
@@ -190,8 +225,25 @@ const char *fbp_last_error(const fbp_plan *plan);
  *   [8] back-projection dynamic shared memory bytes per CTA
  *   [9] filter outputs per thread   [10] filter threads per CTA   [11] filter input slices per row (SB)
  *   [12] filter dynamic shared memory bytes per CTA   [13] kernels launched by fbp_reconstruct at batch = max_batch
+ *   [14] filter units per row (a row is cut into independent units of one warp-width of outputs; 1 for the FFT form)
+ *   [15] SMs of the plan's device
+ *   [16] filter CTAs per launch at batch = max_batch (0 until the filter has run once: it comes from the occupancy query)
+ *   [17] filter kind (1 direct, 2 FFT)   [18] reserved
  */
 int fbp_plan_info(const fbp_plan *plan, int *out, int n);
+
+/*
+ * fbp_set_trace -- optional in-kernel timeline (profiles/: where the microseconds of a step go).  d_marks: DEVICE
+ * array of `capacity` 64-bit words (caller-owned, zero it first), or NULL to switch tracing off.  While set, thread 0
+ * of every CTA of the filter and of the back-projector stores %globaltimer (ns) into its 8-word record:
+ *   filter CTA c          -> d_marks[8 c + s],  s = 0 start, 1 tables and first row staged, 2 partial sums done,
+ *                            3 row reduced, 4 last unit stored (1-3: the CTA's first unit only)
+ *   back-projector CTA c  -> d_marks[8 (F + c) + s],  F = plan_info[16],  s = 0 CTA resident, 1 past the grid
+ *                            dependency, 2 first chunk landed, 3 main loop done, 4 pixels stored
+ * A kernel whose records would not fit in `capacity` is not traced.  One predicated store per mark: the timed
+ * kernels are the product kernels, not an instrumented build.  Not used by the batch pipeline's side streams.
+ */
+fbp_status fbp_set_trace(fbp_plan *plan, unsigned long long *d_marks, long long capacity);
 
 /*
  * fbp_set_profiling / fbp_get_kernel_ms -- optional per-kernel timing of the LAST compute

@@ -9,8 +9,8 @@ from __future__ import annotations
 from .binding import (  # noqa: F401
     EXPORTS, FBP_F32, FBP_F64, FBP_OK, FBP_EINVAL, FBP_ENOMEM, FBP_ECUDA, FBP_EUNSUPPORTED,
     FbpError, load_library,
-    fbp_create, fbp_filter, fbp_backproject, fbp_reconstruct, fbp_reconstruct_host,
-    fbp_destroy, fbp_last_error, fbp_plan_info, fbp_set_profiling, fbp_get_kernel_ms, fbp_metrics, fbp_set_window, fbp_set_angle_weights, WINDOWS, fbp_interpolate_stack, fbp_project,
+    fbp_create, fbp_create_tuned, OPTIONS, fbp_filter, fbp_backproject, fbp_reconstruct, fbp_reconstruct_host,
+    fbp_destroy, fbp_last_error, fbp_plan_info, fbp_set_profiling, fbp_get_kernel_ms, fbp_set_trace, fbp_metrics, fbp_set_window, fbp_set_angle_weights, WINDOWS, fbp_interpolate_stack, fbp_project,
 )
 from .build import build  # noqa: F401
 
@@ -33,13 +33,17 @@ class Plan:
     """RAII wrapper over an ``fbp_plan*`` taking torch CUDA tensors (marshalling only)."""
 
     def __init__(self, angles_rad, n_det, image_n, det_spacing=1.0, pixel_size=0.0, dtype="f32",
-                 max_batch=1, device=-1):
+                 max_batch=1, device=-1, options=None):
         import torch
         self.torch_dtype = torch.float32 if _DTYPES[dtype] == FBP_F32 else torch.float64
         self.n_angles, self.n_det, self.image_n, self.max_batch = len(angles_rad), int(n_det), int(image_n), int(max_batch)
         self.device = torch.device("cuda", torch.cuda.current_device() if device < 0 else device)
-        self.handle = fbp_create(self.n_angles, n_det, angles_rad, det_spacing, image_n, pixel_size,
-                                 _DTYPES[dtype], max_batch, device)
+        if options:
+            self.handle = fbp_create_tuned(self.n_angles, n_det, angles_rad, det_spacing, image_n, pixel_size,
+                                           _DTYPES[dtype], max_batch, device, options)
+        else:
+            self.handle = fbp_create(self.n_angles, n_det, angles_rad, det_spacing, image_n, pixel_size,
+                                     _DTYPES[dtype], max_batch, device)
 
     def info(self) -> dict:
         return fbp_plan_info(self.handle)
@@ -56,28 +60,38 @@ class Plan:
         shape = inner if like.dim() == 2 else (like.shape[0],) + inner
         return torch.empty(shape, dtype=self.torch_dtype, device=like.device)
 
+    def _out(self, out, like, inner):
+        """A caller-supplied result tensor goes to the library as a bare pointer: check it first."""
+        if out is None:
+            return self._empty(like, inner)
+        want = inner if like.dim() == 2 else (like.shape[0],) + inner
+        if (out.dtype != self.torch_dtype or not out.is_cuda or not out.is_contiguous() or out.device != like.device
+                or tuple(out.shape) != tuple(want)):
+            raise ValueError("out must be a contiguous CUDA tensor of the plan dtype, shape %s, on %s" % (list(want), like.device))
+        return out
+
     def filter(self, sino, out=None, stream=None):
         b = self._batch(sino, (self.n_angles, self.n_det))
-        out = self._empty(sino, (self.n_angles, self.n_det)) if out is None else out
+        out = self._out(out, sino, (self.n_angles, self.n_det))
         fbp_filter(self.handle, sino, out, b, stream)
         return out
 
     def backproject(self, filtered, out=None, stream=None):
         b = self._batch(filtered, (self.n_angles, self.n_det))
-        out = self._empty(filtered, (self.image_n, self.image_n)) if out is None else out
+        out = self._out(out, filtered, (self.image_n, self.image_n))
         fbp_backproject(self.handle, filtered, out, b, stream)
         return out
 
     def reconstruct(self, sino, out=None, stream=None):
         b = self._batch(sino, (self.n_angles, self.n_det))
-        out = self._empty(sino, (self.image_n, self.image_n)) if out is None else out
+        out = self._out(out, sino, (self.image_n, self.image_n))
         fbp_reconstruct(self.handle, sino, out, b, stream)
         return out
 
     def project(self, image, out=None, stream=None):
         """Matched forward projector R = B^T (unweighted): image [batch][N][N] -> sinogram [batch][K][D]."""
         b = self._batch(image, (self.image_n, self.image_n))
-        out = self._empty(image, (self.n_angles, self.n_det)) if out is None else out
+        out = self._out(out, image, (self.n_angles, self.n_det))
         fbp_project(self.handle, image, out, b, stream)
         return out
 
@@ -89,6 +103,9 @@ class Plan:
             raise ValueError("expected a contiguous CUDA stack [n_in][N][N] of the plan dtype")
         if out is None:
             out = torch.empty((int(n_out), self.image_n, self.image_n), dtype=self.torch_dtype, device=stack.device)
+        elif (out.dtype != self.torch_dtype or not out.is_cuda or not out.is_contiguous() or out.device != stack.device
+              or tuple(out.shape) != (int(n_out), self.image_n, self.image_n)):
+            raise ValueError("out must be a contiguous CUDA tensor [n_out][N][N] of the plan dtype")
         fbp_interpolate_stack(self.handle, stack, stack.shape[0], out, n_out, stream)
         return out
 
@@ -98,7 +115,7 @@ class Plan:
     def set_angle_weights(self, weights):
         if weights is not None and len(weights) != self.n_angles:
             raise ValueError("expected one weight per angle")
-        fbp_set_angle_weights(self.handle, weights)
+        fbp_set_angle_weights(self.handle, weights, self.n_angles)
 
     def metrics(self, x, y, max_val, c1=-1.0, c2=-1.0, stream=None) -> dict:
         """PSNR / SSIM (eq. 3, 4 of the paper) of two CUDA tensors of the plan dtype; one device-to-host read."""

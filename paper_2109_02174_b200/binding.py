@@ -16,17 +16,23 @@ FBP_OK, FBP_EINVAL, FBP_ENOMEM, FBP_ECUDA, FBP_EUNSUPPORTED = 0, 1, 2, 3, 4
 STATUS_NAMES = {0: "FBP_OK", 1: "FBP_EINVAL", 2: "FBP_ENOMEM", 3: "FBP_ECUDA", 4: "FBP_EUNSUPPORTED"}
 
 EXPORTS = (
-    "fbp_create", "fbp_filter", "fbp_backproject", "fbp_reconstruct", "fbp_reconstruct_host",
+    "fbp_create", "fbp_create_tuned", "fbp_filter", "fbp_backproject", "fbp_reconstruct", "fbp_reconstruct_host",
     "fbp_destroy", "fbp_last_error", "fbp_plan_info", "fbp_set_profiling", "fbp_get_kernel_ms",
-    "fbp_metrics", "fbp_set_window", "fbp_set_angle_weights", "fbp_interpolate_stack", "fbp_project",
+    "fbp_set_trace", "fbp_metrics", "fbp_set_window", "fbp_set_angle_weights", "fbp_interpolate_stack", "fbp_project",
 )
 
 PLAN_INFO_FIELDS = (
     "bp_tile_w", "bp_tile_h", "bp_pixels_per_thread", "bp_angle_splits", "bp_angles_per_chunk",
     "bp_segment_len", "bp_ctas_per_slice", "bp_threads", "bp_smem_bytes",
     "filter_outputs_per_thread", "filter_threads", "filter_input_slices", "filter_smem_bytes",
-    "kernels_per_reconstruct",
+    "kernels_per_reconstruct", "filter_units_per_row", "device_sms", "filter_ctas", "filter_kind",
 )
+
+# keys of fbp_create_tuned (include/fbp.h, fbp_option)
+OPTIONS = {
+    "bp_variant": 1, "bp_splits": 2, "bp_chunk": 3, "filter_r": 4, "filter_sb": 5, "filter_kind": 6,
+    "pipeline": 7, "pipe_group": 8, "pipe_min_batch": 9, "pdl": 10, "host_zero_copy": 11, "bp_even": 13,
+}
 
 _lib = None
 
@@ -51,6 +57,9 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
     lib.fbp_create.argtypes = [ctypes.POINTER(vp), ci, ci, ctypes.POINTER(cd), cd, ci, cd, ci, ci, ci]
     lib.fbp_create.restype = ci
+    lib.fbp_create_tuned.argtypes = [ctypes.POINTER(vp), ci, ci, ctypes.POINTER(cd), cd, ci, cd, ci, ci, ci,
+                                     ctypes.POINTER(ci), ci]
+    lib.fbp_create_tuned.restype = ci
     for name in ("fbp_filter", "fbp_backproject", "fbp_reconstruct", "fbp_reconstruct_host", "fbp_project"):
         fn = getattr(lib, name)
         fn.argtypes = [vp, vp, vp, ci, vp]
@@ -69,6 +78,8 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     lib.fbp_last_error.restype = ctypes.c_char_p
     lib.fbp_plan_info.argtypes = [vp, ctypes.POINTER(ci), ci]
     lib.fbp_plan_info.restype = ci
+    lib.fbp_set_trace.argtypes = [vp, vp, ctypes.c_longlong]
+    lib.fbp_set_trace.restype = ci
     lib.fbp_set_profiling.argtypes = [vp, ci]
     lib.fbp_set_profiling.restype = ci
     lib.fbp_get_kernel_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float)]
@@ -105,17 +116,39 @@ def _stream_handle(stream) -> int:
 
 # ---- the C entry points, same names, same order of arguments -------------------------
 
+def _angle_array(n_angles, angles_rad):
+    """K doubles for the C side, which reads exactly n_angles of them: a shorter list must not get through."""
+    if angles_rad is None:
+        return None
+    vals = [float(a) for a in angles_rad]
+    if len(vals) != int(n_angles):
+        raise ValueError("angles_rad has %d values, n_angles is %d" % (len(vals), int(n_angles)))
+    return (ctypes.c_double * max(len(vals), 1))(*vals)
+
+
 def fbp_create(n_angles, n_det, angles_rad, det_spacing, image_n, pixel_size, dtype, max_batch=1, device=-1):
     """fbp_create of include/fbp.h; returns the opaque plan handle (an int address)."""
     lib = load_library()
-    if angles_rad is None:
-        arr = None
-    else:
-        vals = [float(a) for a in angles_rad]
-        arr = (ctypes.c_double * max(len(vals), 1))(*vals)
+    arr = _angle_array(n_angles, angles_rad)
     plan = ctypes.c_void_p()
     st = lib.fbp_create(ctypes.byref(plan), int(n_angles), int(n_det), arr, float(det_spacing), int(image_n),
                         float(pixel_size), int(dtype), int(max_batch), int(device))
+    _check(lib, None, st)
+    return plan.value
+
+
+def fbp_create_tuned(n_angles, n_det, angles_rad, det_spacing, image_n, pixel_size, dtype, max_batch=1, device=-1,
+                     options=None):
+    """fbp_create_tuned of include/fbp.h; `options` maps option names (OPTIONS) or integer keys to ints."""
+    lib = load_library()
+    arr = _angle_array(n_angles, angles_rad)
+    flat = []
+    for k, v in (options or {}).items():
+        flat += [int(OPTIONS.get(k, k)), int(v)]
+    opts = (ctypes.c_int * max(len(flat), 1))(*flat)
+    plan = ctypes.c_void_p()
+    st = lib.fbp_create_tuned(ctypes.byref(plan), int(n_angles), int(n_det), arr, float(det_spacing), int(image_n),
+                              float(pixel_size), int(dtype), int(max_batch), int(device), opts, len(flat) // 2)
     _check(lib, None, st)
     return plan.value
 
@@ -158,6 +191,11 @@ def fbp_plan_info(plan) -> dict:
     return {PLAN_INFO_FIELDS[i]: int(buf[i]) for i in range(min(n, got))}
 
 
+def fbp_set_trace(plan, d_marks, capacity=0):
+    lib = load_library()
+    _check(lib, plan, lib.fbp_set_trace(plan, _ptr(d_marks), int(capacity)))
+
+
 def fbp_set_profiling(plan, enable: bool):
     lib = load_library()
     _check(lib, plan, lib.fbp_set_profiling(plan, 1 if enable else 0))
@@ -184,12 +222,17 @@ def fbp_set_window(plan, window):
     _check(lib, plan, lib.fbp_set_window(plan, int(WINDOWS.get(window, window))))
 
 
-def fbp_set_angle_weights(plan, weights):
+def fbp_set_angle_weights(plan, weights, n_angles=None):
+    """`n_angles` = the plan's K: the C side reads exactly K doubles, so the length is checked here."""
     lib = load_library()
     if weights is None:
         arr = None
     else:
         vals = [float(w) for w in weights]
+        if n_angles is None:
+            raise ValueError("n_angles (the plan's K) is required with a weight list")
+        if len(vals) != int(n_angles):
+            raise ValueError("expected %d weights, got %d" % (int(n_angles), len(vals)))
         arr = (ctypes.c_double * max(len(vals), 1))(*vals)
     _check(lib, plan, lib.fbp_set_angle_weights(plan, arr))
 

@@ -40,15 +40,11 @@
 #include <cuda_runtime.h>
 #include <cstdint>
 
-#include "fbp_filter.cuh"  // BpEntry
+#include "fbp_entries.cuh"  // entry layout
+#include "fbp_ptx.cuh"      // mbarrier, TMA bulk copy, trace_mark
 
 namespace fbp {
 
-#ifdef FBP_TRACE
-#define FBP_BP_MARK(slot) do { if (threadIdx.x == 0 && blockIdx.x < 4096) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_trace[blockIdx.x * 16 + 8 + (slot)] = t_; } } while (0)
-#else
-#define FBP_BP_MARK(slot) do { } while (0)
-#endif
 
 struct BpParams {
     int n_angles, n_det, image_n;
@@ -60,7 +56,7 @@ struct BpParams {
     int ent_pitch, ent_guard;
     double c_n, c_d;     // (N-1)/2, (D-1)/2
     double scale;        // pi / K
-    const void* recs;    // [tiles][K] AngleRec<T> precomputed by fbp_create (pad = entry offset), or NULL
+    unsigned long long* trace;   // fbp_set_trace: [CTAs][8] %globaltimer marks, or NULL
 };
 
 template <typename T> struct Magic;
@@ -76,55 +72,6 @@ template <> struct Magic<double> {
 };
 
 template <typename T> struct alignas(4 * sizeof(T)) AngleRec { T c, s, b, pad; };
-// the entry offset of a precomputed record travels in `pad` as raw integer bits
-template <typename T> struct RecOffset;
-template <> struct RecOffset<float> {
-    __host__ __device__ static float put(int off) { union { int i; float f; } u; u.i = off; return u.f; }
-    __device__ static long long get(float pad) { return (long long)__float_as_int(pad); }
-};
-template <> struct RecOffset<double> {
-    __host__ __device__ static double put(int off) { union { long long i; double f; } u; u.i = off; return u.f; }
-    __device__ static long long get(double pad) { return __double_as_longlong(pad); }
-};
-
-// ---- PTX wrappers: shared-space addresses, mbarrier, TMA 1-D bulk copy ----------------
-__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void fence_mbar_init()
-{
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(unsigned bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(bar), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void tma_load_1d(unsigned dst, const void* src, unsigned bytes, unsigned bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
-}
-
-
 // ---- the per-update arithmetic: (pixel, mirror pixel) accumulator pair ---------------------
 // fp32: packed pair in one 64-bit register; LDS.128 -> (mids, slopes) as two packed pairs;
 //       t = slopes * (w, w) + mids  (FFMA2, scalar w broadcast);  acc += t  (FADD2).
@@ -205,7 +152,8 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
     const unsigned seg = smem_u32(seg_ptr);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    FBP_BP_MARK(0);
+    const unsigned cta_id = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
+    trace_mark(prm.trace, cta_id, 0);                          // CTA resident
     const bool producer = warp == NW;
     const int wy = warp % WY, wa = producer ? WA : warp / WY;
     const int tile = blockIdx.x;
@@ -232,7 +180,7 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
     // E.  Every thread blocks here (consumers would otherwise spin on their mbarriers and take issue
     // slots from that kernel); a no-op when launched without the attribute.
     asm volatile("griddepcontrol.wait;" ::: "memory");
-    FBP_BP_MARK(1);
+    trace_mark(prm.trace, cta_id, 1);                          // past the grid dependency
 
     PairAcc<T> acc[R];
 #pragma unroll
@@ -252,27 +200,21 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
             for (int a = lane; a < na; a += 32) {
                 AngleRec<T> rc;
                 long long off;            // first staged entry of this angle's row, in entries from the row start
-                if (prm.recs) {
-                    // records precomputed on the host (same fp64 formulas as below): the producer only copies
-                    rc = static_cast<const AngleRec<T>*>(prm.recs)[(size_t)tile * K + a0 + a];
-                    off = RecOffset<T>::get(rc.pad);
+                const double2 cs = cs2[a0 + a];
+                const double ub = x0 * cs.x + y0 * cs.y + prm.c_d;
+                const double umin = ub + fmin(0.0, 31.0 * cs.x) + fmin(0.0, (double)(TH - 1) * cs.y);
+                const double fl = floor(umin) - 1.0;
+                // the window [j0, j0+L) must lie inside the guarded row [-guard, pitch-guard)
+                if (fl >= -(double)prm.ent_guard && fl <= (double)(prm.ent_pitch - prm.ent_guard - L)) {
+                    off = (long long)fl + prm.ent_guard;
+                    rc.c = (T)cs.x; rc.s = (T)cs.y; rc.b = (T)(ub - fl - 0.5);
                 } else {
-                    const double2 cs = cs2[a0 + a];
-                    const double ub = x0 * cs.x + y0 * cs.y + prm.c_d;
-                    const double umin = ub + fmin(0.0, 31.0 * cs.x) + fmin(0.0, (double)(TH - 1) * cs.y);
-                    const double fl = floor(umin) - 1.0;
-                    // the window [j0, j0+L) must lie inside the guarded row [-guard, pitch-guard)
-                    if (fl >= -(double)prm.ent_guard && fl <= (double)(prm.ent_pitch - prm.ent_guard - L)) {
-                        off = (long long)fl + prm.ent_guard;
-                        rc.c = (T)cs.x; rc.s = (T)cs.y; rc.b = (T)(ub - fl - 0.5);
-                    } else {
-                        // the tile projects entirely off the detector at this angle: stage the
-                        // all-zero left guard and pin every pixel to entry 1 of it
-                        off = 0;
-                        rc.c = T(0); rc.s = T(0); rc.b = T(1);
-                    }
-                    rc.pad = T(0);
+                    // the tile projects entirely off the detector at this angle: stage the
+                    // all-zero left guard and pin every pixel to entry 1 of it
+                    off = 0;
+                    rc.c = T(0); rc.s = T(0); rc.b = T(1);
                 }
+                rc.pad = T(0);
                 rec[st * prm.chunk + a] = rc;
                 const uint4* src = Eb + (size_t)(a0 + a) * NP * prm.ent_pitch + off;
 #pragma unroll
@@ -293,7 +235,7 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
             const int st = k % NS;
             const int na = min(prm.chunk, a_end - (a_begin + k * prm.chunk));
             mbar_wait(bar_full + 8u * st, (unsigned)((k / NS) & 1));  // chunk k has landed
-            if (k == 0) FBP_BP_MARK(2);
+            if (k == 0) trace_mark(prm.trace, cta_id, 2);      // first chunk landed (thread 0 is a consumer)
             const AngleRec<T>* rk = rec + st * prm.chunk;
             const unsigned segk = seg + st * stage_stride - Magic<T>::kBits * 16u;  // bits(M) folded in
 #pragma unroll 2
@@ -314,7 +256,7 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
         }
     }
 
-    FBP_BP_MARK(3);
+    trace_mark(prm.trace, cta_id, 3);                          // main loop done
     // ---- in-CTA reduction over the WA angle groups, fixed order g = 0..WA-1 ----
     T va[R], vb[R];
 #pragma unroll
@@ -359,7 +301,7 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
             if (ok_a(r)) img[base_a + (long long)r * N] = va[r] * sc;
             if (ok_b(r)) img[base_b - (long long)r * N] = vb[r] * sc;
         }
-        FBP_BP_MARK(4);
+        trace_mark(prm.trace, cta_id, 4);                      // pixels stored
         return;
     }
 

@@ -73,15 +73,15 @@ stage_image_kernel(const T* __restrict__ x, T* __restrict__ xp, T* __restrict__ 
 // Point symmetry (as in the back-projector): the mirror pixel (N-1-l, N-1-p) has u' = (D-1) - u, so it meets the
 // mirror bin D-1-j with the SAME weight hat(u - j).  A thread therefore owns bin j < ceil(D/2) and its mirror bin
 // and computes the run and its weights once for both.
-// cs2: [K] (cos, sin) * pix/d in fp64.  Grid (ceil(ceil(D/2)/128), K, batch), block 128: thread = bin j.
+// cs2: [K] (cos, sin) * pix/d in fp64.  Grid (bin_blocks * K, 1, batch), bin_blocks = ceil(ceil(D/2)/128), block 128: thread = bin j.
 // xp / xtp: the padded image and its padded transpose (stage_image_kernel).  y: [batch][K][D], fully written.
 template <typename T>
 __global__ void __launch_bounds__(128)
 project_kernel(const T* __restrict__ xp, const T* __restrict__ xtp, T* __restrict__ y,
-               const double2* __restrict__ cs2, ProjParams prm)
+               const double2* __restrict__ cs2, ProjParams prm, int bin_blocks)
 {
-    const int j = blockIdx.x * 128 + threadIdx.x;
-    const int i = blockIdx.y, b = blockIdx.z;
+    const int i = blockIdx.x / bin_blocks, b = blockIdx.z;
+    const int j = (blockIdx.x - i * bin_blocks) * 128 + threadIdx.x;
     const int N = prm.image_n, pitch = N + 2 * prm.pad;
     if (j >= (prm.n_det + 1) / 2) return;
     const int jm = prm.n_det - 1 - j;            // mirror bin (== j for the middle bin of an odd detector)

@@ -1,6 +1,6 @@
 """Small driver for `compute-sanitizer` (memcheck / racecheck / initcheck / synccheck):
 
-    compute-sanitizer --tool racecheck python -m paper_2109_02174_b200.selfcheck
+    compute-sanitizer --tool racecheck python tests/selfcheck.py
 
 Runs every kernel family once on tiny geometries (both dtypes, angle splits on and off, the batch
 pipeline, the host path) and checks that repeated runs are bit-identical.  No oracle here: parity is
@@ -11,6 +11,8 @@ import math
 import os
 import sys
 
+sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+
 
 def main() -> int:
     import numpy as np
@@ -20,19 +22,19 @@ def main() -> int:
 
     pkg.load_library()
     torch.cuda.set_device(0)
-    cases = [  # (N, K, D, batch, env)
+    cases = [  # (N, K, D, batch, options of fbp_create_tuned)
         (40, 24, 61, 1, {}),
-        (33, 10, 48, 2, {"FBP_BP_SPLITS": "3"}),
+        (33, 10, 48, 2, {"bp_splits": 3}),
         (64, 16, 91, 9, {}),                       # batch >= 8: pipelined path
-        (24, 8, 40, 1, {"FBP_FILTER_V": "1"}),
+        (24, 8, 40, 1, {"pdl": 0}),
+        (90, 12, 500, 1, {"filter_sb": 2}),        # two filter units per row
     ]
     for n, k, d, b, env in cases:
-        os.environ.update(env)
-        try:
+        if True:
             ang = [i * math.pi / k for i in range(k)]
             for dt, tdt in (("f32", torch.float32), ("f64", torch.float64)):
                 sino = torch.from_numpy(np.random.default_rng(n + k).standard_normal((b, k, d))).to(tdt).cuda()
-                with pkg.Plan(ang, d, n, dtype=dt, max_batch=b) as plan:
+                with pkg.Plan(ang, d, n, dtype=dt, max_batch=b, options=env) as plan:
                     first = plan.reconstruct(sino).clone()
                     q = plan.filter(sino)
                     two = plan.backproject(q)
@@ -47,15 +49,12 @@ def main() -> int:
                     if not torch.equal(host_out, first.cpu()):
                         print("HOST MISMATCH", n, k, d, b, dt, env)
                         return 1
-        finally:
-            for key in env:
-                os.environ.pop(key, None)
     print("selfcheck ok")
     return 0
 
 
 def soak(runs: int) -> int:
-    """``--soak N``: N reconstructions per case with other work interleaved; every 25th result and the last are
+    """``python tests/selfcheck.py --soak N``: N reconstructions per case with other work interleaved; every 25th result and the last are
     compared bit for bit with the first (the paper's parallel versions differed on every run)."""
     import numpy as np
     import torch
@@ -66,14 +65,13 @@ def soak(runs: int) -> int:
     pkg.load_library()
     torch.cuda.set_device(0)
     bad = 0
-    for cid, dt, batch, env in ((3, "f32", 1, {}), (3, "f64", 1, {}), (3, "f32", 1, {"FBP_BP_SPLITS": "3"}),
+    for cid, dt, batch, env in ((3, "f32", 1, {}), (3, "f64", 1, {}), (3, "f32", 1, {"bp_splits": 3}),
                                 (2, "f32", 12, {}), (1, "f32", 1, {})):
-        os.environ.update(env)
-        try:
+        if True:
             cfg = I.CONFIGS[cid]
             tdt = torch.float32 if dt == "f32" else torch.float64
             sino = torch.from_numpy(np.stack([I.config_slice(cid, s % 3) for s in range(batch)])).to(tdt).cuda()
-            with pkg.Plan(list(I.config_angles(cid)), cfg.n_det, cfg.image_n, dtype=dt, max_batch=batch) as plan:
+            with pkg.Plan(list(I.config_angles(cid)), cfg.n_det, cfg.image_n, dtype=dt, max_batch=batch, options=env) as plan:
                 first = plan.reconstruct(sino).clone()
                 junk = torch.randn(2048, 2048, device="cuda")
                 miss = 0
@@ -86,9 +84,6 @@ def soak(runs: int) -> int:
                 torch.cuda.synchronize()
             print("cfg%d %s batch %d %s: %d runs, %d mismatches" % (cid, dt, batch, env, runs, miss))
             bad += miss
-        finally:
-            for key in env:
-                os.environ.pop(key, None)
     return 1 if bad else 0
 
 

@@ -55,6 +55,28 @@ def test_create_rejects_bad_arguments_before_touching_cuda(lib):
     assert lib.fbp_create(None, 4, 8, ang, 1.0, 8, 1.0, 0, 1, -1) == pkg.FBP_EINVAL
 
 
+def test_create_tuned_rejects_bad_option_lists(lib):
+    ang = (ctypes.c_double * 4)(0.0, 0.5, 1.0, 1.5)
+    plan = ctypes.c_void_p(123)
+    bad_key = (ctypes.c_int * 2)(9999, 1)
+    assert lib.fbp_create_tuned(ctypes.byref(plan), 4, 8, ang, 1.0, 8, 1.0, 0, 1, -1, bad_key, 1) == pkg.FBP_EINVAL
+    assert plan.value is None
+    assert lib.fbp_create_tuned(ctypes.byref(plan), 4, 8, ang, 1.0, 8, 1.0, 0, 1, -1, None, 2) == pkg.FBP_EINVAL
+    assert lib.fbp_create_tuned(ctypes.byref(plan), 4, 8, ang, 1.0, 8, 1.0, 0, 1, -1, bad_key, -1) == pkg.FBP_EINVAL
+    with pytest.raises(ValueError):
+        pkg.fbp_create(5, 8, [0.0, 0.5, 1.0, 1.5], 1.0, 8, 0.0, pkg.FBP_F32)     # the C side would read 5 doubles
+    with pytest.raises(ValueError):
+        pkg.fbp_create_tuned(3, 8, [0.0, 0.5, 1.0, 1.5], 1.0, 8, 0.0, pkg.FBP_F32)
+
+
+def test_library_does_not_read_the_environment():
+    """Behaviour depends on the arguments only (fbp_create_tuned): no getenv in the product sources."""
+    for dirpath, _, files in os.walk(os.path.join(ROOT, "paper_2109_02174_b200", "csrc")):
+        for f in files:
+            src = open(os.path.join(dirpath, f)).read()
+            assert "getenv" not in src and "environ[" not in src and "putenv" not in src, f
+
+
 def test_null_plan_is_rejected_or_ignored(lib):
     assert lib.fbp_filter(None, 16, 32, 1, None) == pkg.FBP_EINVAL
     assert lib.fbp_backproject(None, 16, 32, 1, None) == pkg.FBP_EINVAL

@@ -111,6 +111,7 @@ WINDOW_CASES = [  # (N, K, D, d, batch)
     (130, 31, 185, 1.0, 1),
     (256, 24, 363, 1.0, 1),        # config 2 row length
     (40, 12, 725, 2.0, 1),         # config 3 row length
+    (64, 5, 2897, 1.0, 1),         # config 5 row length: several filter units per row
 ]
 
 
@@ -153,10 +154,12 @@ def test_windowed_cfg3_full_image(fbp, oracle, dt):
     _check_image(a.cpu().numpy(), ref, dt, "cfg3 hann")
 
 
+@pytest.mark.parametrize("b", [2, 9])
 @pytest.mark.parametrize("dt", ["f32", "f64"])
-def test_angle_weights_match_oracle(fbp, oracle, dt):
-    """Non-uniform angles with trapezoid weights; NULL restores pi/K."""
-    n, k, dd, b = 70, 41, 101, 2
+def test_angle_weights_match_oracle(fbp, oracle, dt, b):
+    """Non-uniform angles with trapezoid weights; NULL restores pi/K.
+    b = 9 takes the batch pipeline (filter and back-projection of slice groups on plan-owned streams)."""
+    n, k, dd = 70, 41, 101
     rng = np.random.default_rng(17)
     ang = np.sort(rng.uniform(0.0, math.pi, k))
     edges = np.concatenate([[ang[-1] - math.pi], ang, [ang[0] + math.pi]])
@@ -182,7 +185,9 @@ def test_window_and_weight_error_paths(fbp):
             fbp.fbp_set_window(plan.handle, 9)
         assert ei.value.status == fbp.FBP_EINVAL
         with pytest.raises(fbp.FbpError):
-            fbp.fbp_set_angle_weights(plan.handle, [1.0] * 7 + [float("inf")])
+            fbp.fbp_set_angle_weights(plan.handle, [1.0] * 7 + [float("inf")], 8)
+        with pytest.raises(ValueError):
+            fbp.fbp_set_angle_weights(plan.handle, [1.0] * 7, 8)          # the C side would read 8 doubles
         with pytest.raises(ValueError):
             plan.set_angle_weights([1.0] * 3)
 
@@ -245,7 +250,7 @@ def test_stack_interpolation_of_reconstructed_slices_and_errors(fbp, oracle):
 
 
 def test_selfcheck_driver(fbp):
-    from paper_2109_02174_b200 import selfcheck
+    import selfcheck                     # tests/selfcheck.py (the tests directory is on sys.path under pytest)
     assert selfcheck.main() == 0
 
 

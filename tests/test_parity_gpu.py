@@ -51,8 +51,15 @@ def check_image(gpu, ref, dt, what=""):
     return mx
 
 
-def check_filter(gpu, ref, dt, what="", p_max=None, d=1.0):
-    """p_max = max|P| of the (rounded) input rows the outputs come from (fp32 bound above)."""
+# fp32 filter error measured on B200 with the conditioned sums, as a fraction of max|Q_oracle|.
+# R1 (the n-term bound below) stays the outer bar; these figures, with 2x headroom, make a regression of the
+# conditioning visible long before R1 is reached (at config 5 R1 is only 3x above what is measured).
+RECORDED_F32_FILTER_ERR = {1: 5.0e-7, 2: 8.6e-7, 3: 1.4e-6, 4: 2.5e-6, 5: 1.8e-5}
+
+
+def check_filter(gpu, ref, dt, what="", p_max=None, d=1.0, recorded=None):
+    """p_max = max|P| of the (rounded) input rows the outputs come from (fp32 bound above).
+    recorded: the measured fp32 error of this config relative to max|Q| (RECORDED_F32_FILTER_ERR)."""
     gpu = np.asarray(gpu, dtype=np.float64)
     err = np.abs(gpu - ref).max()
     if dt == "f64":
@@ -62,10 +69,14 @@ def check_filter(gpu, ref, dt, what="", p_max=None, d=1.0):
     n_det = ref.shape[-1]
     bound = math.sqrt(n_det / 2 + 1) * 2.0 ** -24 * 0.5 * p_max / d
     assert err <= bound, "%s filter fp32 abs err %.3e > bound %.3e" % (what, err, bound)
+    if recorded is not None:
+        rel_q = err / np.abs(ref).max()
+        print("%s: fp32 filter error %.3e of max|Q| (recorded %.1e)" % (what, rel_q, recorded))
+        assert rel_q <= 2.0 * recorded, "%s filter fp32 error %.3e of max|Q| > 2 x recorded %.1e" % (what, rel_q, recorded)
     return err / bound
 
 
-def run_case(fbp, oracle, sino64, angles, n, dt, d=1.0, pix=None, what=""):
+def run_case(fbp, oracle, sino64, angles, n, dt, d=1.0, pix=None, what="", recorded=None):
     """Full three-way check of one geometry: filter, back-projection, reconstruct."""
     torch = _torch()
     sino64 = np.asarray(sino64, dtype=np.float64)
@@ -79,7 +90,7 @@ def run_case(fbp, oracle, sino64, angles, n, dt, d=1.0, pix=None, what=""):
         ds = _to_dev(sino_in, dt)
         q_gpu = plan.filter(ds)
         q_ref = oracle.filter_sinogram(sino_ref, d)
-        check_filter(q_gpu.cpu().numpy(), q_ref, dt, what, np.abs(sino_ref).max(), d)
+        check_filter(q_gpu.cpu().numpy(), q_ref, dt, what, np.abs(sino_ref).max(), d, recorded)
         # back-projection alone, fed the oracle's Q rounded to the dtype
         q_in = q_ref.astype(_np_dtype(dt))
         f_ref_bp = oracle.backproject(q_in.astype(np.float64), angles, n, d, pix)
@@ -101,7 +112,8 @@ def run_case(fbp, oracle, sino64, angles, n, dt, d=1.0, pix=None, what=""):
 @pytest.mark.parametrize("cfg_id,dt", [(1, "f32"), (2, "f32"), (3, "f32"), (3, "f64"), (1, "f64")])
 def test_configs_full_images(fbp, oracle, cfg_id, dt):
     cfg = I.CONFIGS[cfg_id]
-    run_case(fbp, oracle, I.config_sinogram(cfg_id), I.config_angles(cfg_id), cfg.image_n, dt, what=cfg.name)
+    run_case(fbp, oracle, I.config_sinogram(cfg_id), I.config_angles(cfg_id), cfg.image_n, dt, what=cfg.name,
+             recorded=RECORDED_F32_FILTER_ERR[cfg_id])
 
 
 ODD_CASES = [
@@ -144,51 +156,49 @@ def _sample_pixels(n, count, seed):
 
 
 @pytest.mark.parametrize("dt", ["f32", "f64"])
-def test_cfg5_full_size_sampled(fbp, oracle, dt):
-    """2048^2 x 1800 x 2897 in the launch configuration bench.py uses; the oracle checks
-    sampled filter rows and sampled pixels one by one."""
+def test_cfg5_full_image(fbp, oracle, dt):
+    """2048^2 x 1800 x 2897 in the launch configuration bench.py uses: every filter row and EVERY pixel against the
+    oracle (the oracle filters and back-projects the whole slice itself; nothing the CUDA path produced is ever an
+    oracle input); DR over the full image.  This is the launch that uses the 32x32-tile back-projector."""
     cfg = I.CONFIGS[5]
     ang = I.config_angles(5)
     sino_in = I.config_slice(5).astype(_np_dtype(dt))
     sino_ref = sino_in.astype(np.float64)
     plan = fbp.Plan(list(ang), cfg.n_det, cfg.image_n, dtype=dt, max_batch=1)
     try:
+        assert plan.info()["bp_tile_h"] == 32
         ds = _to_dev(sino_in, dt)
         q_gpu = plan.filter(ds).cpu().numpy()
-        rows_f = np.array([0, 1, 449, 900, 1234, 1799], dtype=np.int32)
-        q_rows = oracle.filter_rows(sino_ref, rows_f)
-        check_filter(q_gpu[rows_f], q_rows, dt, "cfg5", np.abs(sino_ref).max())
-        # whole chain on sampled pixels: the oracle filters the full sinogram itself (nothing
-        # the CUDA path produced is ever an oracle input) and back-projects the samples; DR
-        # is taken over the oracle's samples.
         f_gpu = plan.reconstruct(ds).cpu().numpy()
-        rr, cc = _sample_pixels(cfg.image_n, 3000, 55)
         q_ref = oracle.filter_sinogram(sino_ref)
-        check_filter(q_gpu, q_ref, dt, "cfg5 all rows", np.abs(sino_ref).max())
-        f_ref = oracle.backproject_pixels(q_ref, ang, cfg.image_n, rr, cc)
-        check_image(f_gpu[rr, cc], f_ref, dt, "cfg5 sampled")
+        check_filter(q_gpu, q_ref, dt, "cfg5 all rows", np.abs(sino_ref).max(), recorded=RECORDED_F32_FILTER_ERR[5])
+        f_ref = oracle.backproject(q_ref, ang, cfg.image_n)
+        check_image(f_gpu, f_ref, dt, "cfg5 full image")
     finally:
         plan.close()
 
 
-def test_cfg4_batch_sampled(fbp, oracle):
-    """64 slices x 512^2 x 720 in one launch; three slices checked on sampled pixels, one in full."""
+def test_cfg4_batch_every_slice(fbp, oracle):
+    """64 slices x 512^2 x 720 through the batch pipeline, as bench.py --config 4 launches it: every slice, every
+    filter row and every pixel against the oracle, DR per slice."""
     cfg = I.CONFIGS[4]
     ang = I.config_angles(4)
     sino_in = I.config_sinogram(4).astype(np.float32)
     plan = fbp.Plan(list(ang), cfg.n_det, cfg.image_n, dtype="f32", max_batch=cfg.batch)
     try:
+        assert plan.info()["kernels_per_reconstruct"] > 2 and plan.info()["bp_tile_h"] == 32
         ds = _to_dev(sino_in, "f32")
         q_gpu = plan.filter(ds).cpu().numpy()
         f_gpu = plan.reconstruct(ds).cpu().numpy()
-        for s in (0, 37, 63):
-            q_ref = oracle.filter_sinogram(sino_in[s].astype(np.float64))
-            check_filter(q_gpu[s], q_ref, "f32", "cfg4 s%d" % s, np.abs(sino_in[s]).max())
-            rr, cc = _sample_pixels(cfg.image_n, 2000, 400 + s)
-            f_ref = oracle.backproject_pixels(q_ref, ang, cfg.image_n, rr, cc)
-            check_image(f_gpu[s][rr, cc], f_ref, "f32", "cfg4 s%d" % s)
-        f_full = oracle.reconstruct(sino_in[5].astype(np.float64), ang, cfg.image_n)
-        check_image(f_gpu[5], f_full, "f32", "cfg4 s5 full")
+        for s0 in range(0, cfg.batch, 8):
+            sl = slice(s0, s0 + 8)
+            q_ref = oracle.filter_sinogram(sino_in[sl].astype(np.float64))
+            f_ref = oracle.backproject(q_ref, ang, cfg.image_n)
+            for i in range(8):
+                s = s0 + i
+                check_filter(q_gpu[s], q_ref[i], "f32", "cfg4 s%d" % s, np.abs(sino_in[s]).max(),
+                             recorded=RECORDED_F32_FILTER_ERR[4])
+                check_image(f_gpu[s], f_ref[i], "f32", "cfg4 s%d" % s)
     finally:
         plan.close()
 
@@ -216,15 +226,13 @@ def test_bit_identical_across_runs(fbp, dt):
 
 @pytest.mark.parametrize("splits", [1, 2, 5, 7])
 @pytest.mark.parametrize("variant", [0, 1, 2])
-def test_angle_splits_and_tile_variants(fbp, oracle, splits, variant, monkeypatch):
-    monkeypatch.setenv("FBP_BP_SPLITS", str(splits))
-    monkeypatch.setenv("FBP_BP_VARIANT", str(variant))
-    monkeypatch.setenv("FBP_BP_CHUNK", "13")
+def test_angle_splits_and_tile_variants(fbp, oracle, splits, variant):
+    opts = {"bp_splits": splits, "bp_variant": variant, "bp_chunk": 13}
     n, k, dd = 100, 45, 150
     ang = I.uniform_angles(k)
     for dt in ("f32", "f64"):
         q = I.random_sinogram(9, 2, k, dd).astype(_np_dtype(dt))
-        plan = fbp.Plan(list(ang), dd, n, dtype=dt, max_batch=2)
+        plan = fbp.Plan(list(ang), dd, n, dtype=dt, max_batch=2, options=opts)
         try:
             assert plan.info()["bp_angle_splits"] == splits
             f = plan.backproject(_to_dev(q, dt)).cpu().numpy()
@@ -284,7 +292,7 @@ def test_profiling_hooks(fbp):
 
 @pytest.mark.parametrize("dt", ["f32", "f64"])
 @pytest.mark.parametrize("group", [0, 3, 16])
-def test_batch_pipeline_is_bit_identical_to_sequential(fbp, oracle, dt, group, monkeypatch):
+def test_batch_pipeline_is_bit_identical_to_sequential(fbp, oracle, dt, group):
     """fbp_reconstruct on a stack overlaps filter(group g+1) with back-projection(group g) on plan-owned
     streams; the result must be the bytes of the sequential path, at any group size."""
     torch = _torch()
@@ -292,12 +300,11 @@ def test_batch_pipeline_is_bit_identical_to_sequential(fbp, oracle, dt, group, m
     ang = I.uniform_angles(k)
     sino = I.random_sinogram(5, b, k, dd).astype(_np_dtype(dt))
     ds = _to_dev(sino, dt)
-    monkeypatch.setenv("FBP_PIPE", "0")
-    with fbp.Plan(list(ang), dd, n, dtype=dt, max_batch=b) as seq:
+    with fbp.Plan(list(ang), dd, n, dtype=dt, max_batch=b, options={"pipeline": 0, "bp_splits": 1}) as seq:
+        assert seq.info()["kernels_per_reconstruct"] == 2
         want = seq.reconstruct(ds).clone()
-    monkeypatch.setenv("FBP_PIPE", "1")
-    monkeypatch.setenv("FBP_PIPE_GROUP", str(group))
-    with fbp.Plan(list(ang), dd, n, dtype=dt, max_batch=b) as pipe:
+    with fbp.Plan(list(ang), dd, n, dtype=dt, max_batch=b, options={"pipeline": 1, "pipe_group": group, "bp_splits": 1}) as pipe:
+        assert pipe.info()["kernels_per_reconstruct"] > 2
         got = pipe.reconstruct(ds)
         junk = torch.randn(2048, 2048, device="cuda")
         (junk @ junk).sum().item()
@@ -310,13 +317,29 @@ def test_batch_pipeline_is_bit_identical_to_sequential(fbp, oracle, dt, group, m
 
 
 @pytest.mark.parametrize("dt", ["f32", "f64"])
-def test_first_generation_filter_kernel_still_matches(fbp, oracle, dt, monkeypatch):
-    """FBP_FILTER_V=1 selects the one-parity filter kernel kept as the fallback for rows that do not fit the
-    paired kernel's shared-memory layout; it must meet the same tolerances."""
-    monkeypatch.setenv("FBP_FILTER_V", "1")
-    cfg = I.CONFIGS[2]
-    run_case(fbp, oracle, I.config_sinogram(2), I.config_angles(2), cfg.image_n, dt, what="cfg2 filter v1")
-    run_case(fbp, oracle, I.random_sinogram(31, 2, 9, 70), I.uniform_angles(9), 45, dt, 0.5, 0.5, what="odd filter v1")
+@pytest.mark.parametrize("opts", [{"filter_sb": 1}, {"filter_sb": 3}, {"filter_sb": 8}, {"filter_r": 10}, {"filter_r": 14},
+                                  {"pdl": 0}])
+def test_filter_decompositions_match_oracle(fbp, oracle, dt, opts):
+    """The row filter cuts a row into mirrored units of one warp-width (fbp_filter3.cuh): other group sizes R and other
+    numbers of input slices must meet the same tolerances, on rows of 1, 2 and several units, and launching without
+    programmatic dependent launch must not change a byte."""
+    for n, k, dd, d in ((45, 9, 70, 0.5), (96, 7, 501, 1.0), (64, 5, 1203, 1.0)):
+        sino = I.random_sinogram(31 + dd, 2, k, dd)
+        ang = I.uniform_angles(k)
+        sino_in = sino.astype(_np_dtype(dt))
+        with fbp.Plan(list(ang), dd, n, det_spacing=d, dtype=dt, max_batch=2, options=opts) as plan:
+            ds = _to_dev(sino_in, dt)
+            q = plan.filter(ds)
+            f = plan.reconstruct(ds)
+            f2 = plan.backproject(q)
+            _torch().cuda.synchronize()
+            assert _torch().equal(f, f2)
+        q_ref = oracle.filter_sinogram(sino_in.astype(np.float64), d)
+        check_filter(q.cpu().numpy(), q_ref, dt, "units %s D=%d" % (opts, dd), np.abs(sino_in).max(), d)
+        check_image(f.cpu().numpy(), oracle.reconstruct(sino_in.astype(np.float64), ang, n, d), dt, "units %s D=%d" % (opts, dd))
+        if "pdl" in opts:
+            with fbp.Plan(list(ang), dd, n, det_spacing=d, dtype=dt, max_batch=2) as plain:
+                assert _torch().equal(plain.reconstruct(ds), f)
 
 
 def test_long_rows_and_many_angles(fbp, oracle):
