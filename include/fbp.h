@@ -165,7 +165,8 @@ fbp_status fbp_metrics(fbp_plan *plan, const void *d_x, const void *d_y, long lo
  *   FBP_WINDOW_HAMMING      W = 0.54 + 0.46 cos(2 pi f)
  *   FBP_WINDOW_HANN         W = 0.5 + 0.5 cos(2 pi f)
  * Applies to fbp_filter and fbp_reconstruct from the next call on.  Synchronous: waits for the device,
- * rebuilds and uploads the tap tables.  FBP_EUNSUPPORTED if the row is too long for the dense kernel.
+ * rebuilds and uploads the tap tables (FFT form: the DFT of the taps' running sum).  FBP_EUNSUPPORTED if the
+ * plan runs the direct form and the row is too long for its dense kernel.
  */
 typedef enum {
     FBP_WINDOW_RAMLAK = 0,
@@ -223,12 +224,13 @@ const char *fbp_last_error(const fbp_plan *plan);
  *   [4] angles staged per shared-memory chunk   [5] staged segment length (entries per angle)
  *   [6] back-projection CTAs per slice   [7] back-projection threads per CTA
  *   [8] back-projection dynamic shared memory bytes per CTA
- *   [9] filter outputs per thread   [10] filter threads per CTA   [11] filter input slices per row (SB)
+ *   [9] filter outputs per thread (direct form) / points per thread and pass (FFT form)   [10] filter threads per CTA
+ *   [11] filter input slices per row (SB; 0 for the FFT form)
  *   [12] filter dynamic shared memory bytes per CTA   [13] kernels launched by fbp_reconstruct at batch = max_batch
  *   [14] filter units per row (a row is cut into independent units of one warp-width of outputs; 1 for the FFT form)
  *   [15] SMs of the plan's device
  *   [16] filter CTAs per launch at batch = max_batch (0 until the filter has run once: it comes from the occupancy query)
- *   [17] filter kind (1 direct, 2 FFT)   [18] reserved
+ *   [17] filter kind (1 direct, 2 FFT)   [18] transform length N of the FFT form (0 for the direct form)
  */
 int fbp_plan_info(const fbp_plan *plan, int *out, int n);
 

@@ -26,6 +26,7 @@ PLAN_INFO_FIELDS = (
     "bp_segment_len", "bp_ctas_per_slice", "bp_threads", "bp_smem_bytes",
     "filter_outputs_per_thread", "filter_threads", "filter_input_slices", "filter_smem_bytes",
     "kernels_per_reconstruct", "filter_units_per_row", "device_sms", "filter_ctas", "filter_kind",
+    "fft_length",
 )
 
 # keys of fbp_create_tuned (include/fbp.h, fbp_option)

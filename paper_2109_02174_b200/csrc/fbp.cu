@@ -18,6 +18,7 @@
 
 #include "fbp_backproject.cuh"
 #include "fbp_filter3.cuh"
+#include "fbp_fft.cuh"
 #include "fbp_metrics.cuh"
 #include "fbp_stack.cuh"
 #include "fbp_project.cuh"
@@ -69,6 +70,15 @@ struct fbp_plan {
         void* d_u = nullptr;    // [2][tab_len] dtype: UA | UB
         void* d_rho = nullptr;  // [D] dtype: conditioning term
     } f3[2];
+    // FFT-form filter (fbp_fft.cuh)
+    struct Fft {
+        bool ok = false;        // 2D <= 8192: the transform fits the kernel's instantiations
+        int p = 0, threads = 0, smem = 0, buf_bytes = 0, grid_cap = 0;
+        bool tab_smem = false;  // the table is staged in shared memory (it fits beside the transform buffer)
+        void* d_tab = nullptr;  // complex dtype: per-pass twiddles [fft_tw_total(p)], then [N] the DFT of the circular
+                                // kernel of the current window, / (d N)
+    } fft;
+    int filter_kind = 1;        // 1 direct form, 2 FFT form
     int window = 0;             // fbp_set_window; 0 = Ram-Lak
     void* d_xt = nullptr;       // 2 x [max_batch][N][N + 2 pad] dtype: padded image and padded transpose for fbp_project
     void* d_wrow = nullptr;     // [K] dtype: angle weight / (pi/K) (fbp_set_angle_weights); NULL = uniform
@@ -214,6 +224,90 @@ void configure_filter3(fbp_plan* p, bool dense)
     c.smem = (int)(elems * p->esize + 16 + 16);
     c.ok = c.smem <= 200 * 1024;
     c.grid_cap = 0;
+}
+
+// ---- FFT-form filter configuration and tables (fbp_fft.cuh) -------------------------------
+void configure_fft(fbp_plan* p)
+{
+    fbp_plan::Fft& c = p->fft;
+    int pw = 6;
+    while ((1 << pw) < 2 * p->D && pw < 20) ++pw;          // N = 2^pw >= 2 D (no wrap-around of the lags -D .. D-1), >= 64
+    c.p = pw;
+    c.ok = pw <= 13;
+    if (!c.ok) return;
+    const int n = 1 << pw, shift = p->dtype == FBP_F32 ? 5 : 4;
+    c.threads = std::max(32, n / 16);
+    const size_t fft_bytes = (size_t)(n + (n >> shift)) * 2 * p->esize;
+    const size_t row_bytes = 2 * (size_t)(p->bp.ent_pitch + 2) * p->esize;
+    c.buf_bytes = (int)((std::max(fft_bytes, row_bytes) + 15) / 16 * 16);
+    const size_t tab_bytes = (size_t)(fbp::fft_tw_total(pw) + n) * 2 * p->esize;
+    c.tab_smem = 16 + c.buf_bytes + tab_bytes <= 110 * 1024;     // at least two CTAs per SM
+    c.smem = 16 + c.buf_bytes + (c.tab_smem ? (int)tab_bytes : 0);
+    c.grid_cap = 0;
+    if (c.smem > 200 * 1024) c.ok = false;
+}
+
+// in-place radix-2 FFT in long double (host; N a power of two): the kernel's DFT is computed once per window
+void host_fft(std::vector<long double>& re, std::vector<long double>& im)
+{
+    const size_t n = re.size();
+    for (size_t i = 1, j = 0; i < n; ++i) {
+        size_t bit = n >> 1;
+        for (; j & bit; bit >>= 1) j ^= bit;
+        j ^= bit;
+        if (i < j) { std::swap(re[i], re[j]); std::swap(im[i], im[j]); }
+    }
+    for (size_t len = 2; len <= n; len <<= 1) {
+        for (size_t k = 0; k < len / 2; ++k) {
+            const long double ang = -2.0L * kPiL * (long double)k / (long double)len;
+            const long double wr = std::cos(ang), wi = std::sin(ang);
+            for (size_t i = k; i < n; i += len) {
+                const size_t j = i + len / 2;
+                const long double tr = re[j] * wr - im[j] * wi, ti = re[j] * wi + im[j] * wr;
+                re[j] = re[i] - tr; im[j] = im[i] - ti;
+                re[i] += tr; im[i] += ti;
+            }
+        }
+    }
+}
+
+// Per-pass twiddles (once) and the DFT of the circular kernel c[l mod N] = g[l] / (d N), l = -D .. D-1, where
+// g[l] = sum_{m <= l} h_W[m]: h_W is even and sums to zero (|f| W(f) vanishes at f = 0), so g[-1] = -h_W[0]/2 and
+// every other g[l] follows by adding or subtracting finitely many closed-form taps.
+template <typename T>
+cudaError_t upload_fft_tables(fbp_plan* p, int window, bool twiddles)
+{
+    fbp_plan::Fft& c = p->fft;
+    const int n = 1 << c.p, D = p->D, ntw = fbp::fft_tw_total(c.p);
+    cudaError_t e;
+    if (!c.d_tab && (e = cudaMalloc(&c.d_tab, sizeof(T) * 2 * (size_t)(ntw + n))) != cudaSuccess) return e;
+    if (twiddles) {
+        // [pass][r - 1][k] = exp(-2 pi i k r / (NS R)): the order in which the lanes of a pass read them
+        std::vector<T> w(2 * (size_t)ntw);
+        size_t o = 0;
+        int ns = 16;
+        for (int pass = 1; pass < fbp::fft_n_passes(c.p); ++pass) {
+            const int R = fbp::fft_radix(c.p, pass);
+            for (int r = 1; r < R; ++r)
+                for (int k = 0; k < ns; ++k) {
+                    const long double ang = 2.0L * kPiL * (long double)k * (long double)r / ((long double)ns * (long double)R);
+                    w[o++] = (T)std::cos(ang); w[o++] = (T)(-std::sin(ang));
+                }
+            ns *= R;
+        }
+        if ((e = cudaMemcpy(c.d_tab, w.data(), sizeof(T) * w.size(), cudaMemcpyHostToDevice)) != cudaSuccess) return e;
+    }
+    std::vector<long double> re((size_t)n, 0.0L), im((size_t)n, 0.0L);
+    const long double scale = 1.0L / ((long double)p->d * (long double)n);
+    long double g = -0.5L * window_tap(window, 0);           // g[-1]
+    re[(size_t)(n - 1)] = g * scale;
+    for (long long l = -2; l >= -(long long)D; --l) { g -= window_tap(window, l + 1); re[(size_t)(n + l)] = g * scale; }
+    g = -0.5L * window_tap(window, 0);
+    for (long long l = 0; l <= (long long)D - 1; ++l) { g += window_tap(window, l); re[(size_t)l] = g * scale; }
+    host_fft(re, im);
+    std::vector<T> gt(2 * (size_t)n);
+    for (int k = 0; k < n; ++k) { gt[2 * k] = (T)re[k]; gt[2 * k + 1] = (T)im[k]; }
+    return cudaMemcpy(static_cast<T*>(c.d_tab) + 2 * (size_t)ntw, gt.data(), sizeof(T) * 2 * (size_t)n, cudaMemcpyHostToDevice);
 }
 
 // ---- back-projection launch configuration ------------------------------------------
@@ -406,9 +500,53 @@ cudaError_t launch_filter3_r(fbp_plan* p, const void* sino, void* filt, void* en
     return cudaGetLastError();
 }
 
+template <typename T, int P, bool TSMEM>
+cudaError_t launch_fft_p(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st)
+{
+    fbp_plan::Fft& c = p->fft;
+    auto kern = fbp::fft_filter_kernel<T, P, TSMEM>;
+    static bool smem_open[kMaxDevices] = {};
+    if (cudaError_t e = allow_max_smem(kern, smem_open, p->device); e != cudaSuccess) return e;
+    if (c.grid_cap == 0) {
+        int per_sm = 0;
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, c.threads, c.smem);
+        if (e != cudaSuccess) return e;
+        if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+        c.grid_cap = per_sm * p->num_sm;
+    }
+    fbp::FftParams f{batch, p->K, p->D, (p->K + 1) / 2, p->bp.ent_pitch, p->bp.ent_guard, c.buf_bytes, nullptr};
+    const long long work = (long long)batch * f.pairs_per_slice;
+    const int grid = (int)std::min<long long>(work, c.grid_cap);
+    if (p->d_trace && 8LL * grid <= p->trace_cap) f.trace = p->d_trace;
+    kern<<<grid, c.threads, c.smem, st>>>(static_cast<const T*>(sino), static_cast<T*>(filt), static_cast<uint4*>(ent),
+                                          static_cast<const fbp::Cx<T>*>(c.d_tab), static_cast<const T*>(p->d_wrow), f);
+    return cudaGetLastError();
+}
+
+template <typename T, bool TSMEM>
+cudaError_t launch_fft_t(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st)
+{
+    switch (p->fft.p) {
+        case 6: return launch_fft_p<T, 6, TSMEM>(p, sino, filt, ent, batch, st);
+        case 7: return launch_fft_p<T, 7, TSMEM>(p, sino, filt, ent, batch, st);
+        case 8: return launch_fft_p<T, 8, TSMEM>(p, sino, filt, ent, batch, st);
+        case 9: return launch_fft_p<T, 9, TSMEM>(p, sino, filt, ent, batch, st);
+        case 10: return launch_fft_p<T, 10, TSMEM>(p, sino, filt, ent, batch, st);
+        case 11: return launch_fft_p<T, 11, TSMEM>(p, sino, filt, ent, batch, st);
+        case 12: return launch_fft_p<T, 12, TSMEM>(p, sino, filt, ent, batch, st);
+        default: return launch_fft_p<T, 13, TSMEM>(p, sino, filt, ent, batch, st);
+    }
+}
+template <typename T>
+cudaError_t launch_fft(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st)
+{
+    return p->fft.tab_smem ? launch_fft_t<T, true>(p, sino, filt, ent, batch, st) : launch_fft_t<T, false>(p, sino, filt, ent, batch, st);
+}
+
 template <typename T>
 cudaError_t launch_filter(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st)
 {
+    if (p->filter_kind == 2) return launch_fft<T>(p, sino, filt, ent, batch, st);
     if (p->window != 0) {
         switch (p->f3[1].r) {
             case 5: return launch_filter3_r<T, 5, true>(p, sino, filt, ent, batch, st);
@@ -433,6 +571,15 @@ cudaError_t launch_entries(fbp_plan* p, const void* filt, int batch, cudaStream_
     kern<<<batch * p->K, 256, smem, st>>>(static_cast<const T*>(filt), static_cast<uint4*>(p->d_ent), p->D,
                                           p->bp.ent_pitch, p->bp.ent_guard, static_cast<const T*>(p->d_wrow), p->K);
     return cudaGetLastError();
+}
+
+// filter CTAs per launch at batch = max_batch (plan_info[16]); 0 until the filter has run once
+long long filter_ctas(const fbp_plan* p)
+{
+    if (p->filter_kind == 2)
+        return p->fft.grid_cap > 0 ? std::min<long long>((long long)p->max_batch * ((p->K + 1) / 2), p->fft.grid_cap) : 0;
+    const fbp_plan::F3& f = p->f3[p->window != 0 ? 1 : 0];
+    return f.grid_cap > 0 ? std::min<long long>((long long)p->max_batch * p->K * f.prm.n_units, f.grid_cap) : 0;
 }
 
 template <typename T, int R, int WY, int WA>
@@ -461,8 +608,7 @@ cudaError_t launch_bp_v(fbp_plan* p, void* image, int batch, cudaStream_t st, in
     // trace records of the back-projector follow the filter's (fbp_set_trace)
     prm.trace = nullptr;
     if (p->d_trace) {
-        const fbp_plan::F3& f = p->f3[p->window != 0 ? 1 : 0];
-        const long long f_ctas = std::min<long long>((long long)p->max_batch * p->K * f.prm.n_units, f.grid_cap);   // plan_info[16]
+        const long long f_ctas = filter_ctas(p);   // plan_info[16]
         const long long b_ctas = (long long)cfg.gridDim.x * cfg.gridDim.y * cfg.gridDim.z;
         if (8 * (f_ctas + b_ctas) <= p->trace_cap) prm.trace = p->d_trace + 8 * f_ctas;
     }
@@ -643,11 +789,17 @@ fbp_status create_impl(fbp_plan** out, int n_angles, int n_det, const double* an
     configure_bp(p, cs);
     configure_filter3(p, false);   // after configure_bp: needs the entry pitch
     configure_filter3(p, true);
+    configure_fft(p);
+    // FFT form wherever the transform fits (it does ~D / (10 log2 D) times less work than the direct form and
+    // is better conditioned in fp32); the direct form for longer rows, or on request
+    p->filter_kind = tune.filter_kind == 1 ? 1 : (tune.filter_kind == 2 ? 2 : (p->fft.ok ? 2 : 1));
+    if (p->filter_kind == 2 && !p->fft.ok) p->filter_kind = p->f3[0].ok ? 1 : 2;
+    if (p->filter_kind == 1 && !p->f3[0].ok && p->fft.ok) p->filter_kind = 2;
     p->use_pdl = tune.pdl != 0;
     p->host_zero_copy = tune.host_zero_copy != 0;
 
     auto bail = [&](fbp_status st) { std::string m = p->err; fbp_destroy(p); g_create_error = m; return st; };
-    if (!p->f3[0].ok) { p->err = "n_det too large for the shared-memory row filter"; return bail(FBP_EUNSUPPORTED); }
+    if (!p->f3[0].ok && !p->fft.ok) { p->err = "n_det too large for the shared-memory row filter"; return bail(FBP_EUNSUPPORTED); }
     if (p->bp_smem > 220 * 1024) { p->err = "pixel_size/det_spacing too large for the staged segment"; return bail(FBP_EUNSUPPORTED); }
 
     DeviceGuard guard(device);
@@ -660,7 +812,10 @@ fbp_status create_impl(fbp_plan** out, int n_angles, int n_det, const double* an
     } while (0)
     FBP_TRY(cudaMalloc(&p->d_cs2, sizeof(double2) * (size_t)n_angles));
     FBP_TRY(cudaMemcpy(p->d_cs2, cs.data(), sizeof(double2) * (size_t)n_angles, cudaMemcpyHostToDevice));
-    FBP_TRY(dtype == FBP_F32 ? upload_filter3_tables<float>(p, false, 0) : upload_filter3_tables<double>(p, false, 0));
+    if (p->filter_kind == 1)
+        FBP_TRY(dtype == FBP_F32 ? upload_filter3_tables<float>(p, false, 0) : upload_filter3_tables<double>(p, false, 0));
+    else
+        FBP_TRY(dtype == FBP_F32 ? upload_fft_tables<float>(p, 0, true) : upload_fft_tables<double>(p, 0, true));
     // entries: zero-filled once, so that the guard entries (never written by the filter) read as zeros
     const size_t ent_bytes = 4 * p->esize * (size_t)max_batch * n_angles * p->bp.ent_pitch;
     FBP_TRY(cudaMalloc(&p->d_ent, ent_bytes));
@@ -736,6 +891,7 @@ void fbp_destroy(fbp_plan* p)
         cudaFree(p->d_cs2); cudaFree(p->d_ent); cudaFree(p->d_part); cudaFree(p->d_tickets);
         cudaFree(p->d_hsino); cudaFree(p->d_himg); cudaFree(p->d_mscratch); cudaFree(p->d_wrow); cudaFree(p->d_xt);
         for (int i = 0; i < 2; ++i) { cudaFree(p->f3[i].d_u); cudaFree(p->f3[i].d_rho); }
+        cudaFree(p->fft.d_tab);
         for (int i = 0; i < 4; ++i) if (p->ev[i]) cudaEventDestroy(p->ev[i]);
         if (p->st_f) { cudaStreamSynchronize(p->st_f); cudaStreamDestroy(p->st_f); }
         for (int i = 0; i < 2; ++i) if (p->st_b[i]) { cudaStreamSynchronize(p->st_b[i]); cudaStreamDestroy(p->st_b[i]); }
@@ -818,7 +974,7 @@ fbp_status fbp_reconstruct_host(fbp_plan* p, const void* h_sino, void* h_image, 
         const void* sino_src = p->d_hsino;
         {
             cudaPointerAttributes attr{};
-            if (p->host_zero_copy && sino_bytes * batch <= ((size_t)8 << 20) && p->f3[p->window != 0 ? 1 : 0].prm.n_units == 1 &&
+            if (p->host_zero_copy && sino_bytes * batch <= ((size_t)8 << 20) && p->filter_kind == 1 && p->f3[p->window != 0 ? 1 : 0].prm.n_units == 1 &&
                 cudaPointerGetAttributes(&attr, h_sino) == cudaSuccess && attr.type == cudaMemoryTypeHost &&
                 attr.devicePointer != nullptr && aligned16(attr.devicePointer))
                 sino_src = attr.devicePointer;
@@ -940,6 +1096,16 @@ fbp_status fbp_set_window(fbp_plan* p, fbp_window window)
 {
     if (!p) return FBP_EINVAL;
     if ((int)window < 0 || (int)window > (int)FBP_WINDOW_HANN) return fail(p, FBP_EINVAL, "unknown window");
+    if (p->filter_kind == 2) {
+        // the FFT form treats every window alike: only the kernel's DFT changes
+        DeviceGuard guard(p->device);
+        FBP_CUDA(p, cudaDeviceSynchronize());      // nothing of this plan may be in flight while its tables change
+        cudaError_t e = p->dtype == FBP_F32 ? upload_fft_tables<float>(p, (int)window, false)
+                                            : upload_fft_tables<double>(p, (int)window, false);
+        if (e != cudaSuccess) return cuda_fail(p, e, "window tables");
+        p->window = (int)window;
+        return FBP_OK;
+    }
     if (window == FBP_WINDOW_RAMLAK) { p->window = 0; return FBP_OK; }
     if (!p->f3[1].ok) return fail(p, FBP_EUNSUPPORTED, "n_det too large for the dense (windowed) row filter");
     DeviceGuard guard(p->device);
@@ -985,12 +1151,11 @@ int fbp_plan_info(const fbp_plan* p, int* out, int n)
         launches = 2 * ((p->max_batch + group - 1) / group);
     }
     const fbp_plan::F3& f = p->f3[p->window != 0 ? 1 : 0];
-    const long long f_work = (long long)p->max_batch * p->K * f.prm.n_units;
-    const int f_grid = f.grid_cap > 0 ? (int)std::min<long long>(f_work, f.grid_cap) : 0;   // 0 until the filter has run once
+    const bool fft = p->filter_kind == 2;
     const int v[19] = {p->bp_tw, p->bp_th, p->bp_r, p->bp_splits, p->bp_chunk, p->bp_seg,
                        p->bp.tiles_x * p->bp.tiles_y * p->bp_splits, p->bp_threads, p->bp_smem,
-                       2 * f.r, f.threads, f.prm.n_sb, f.smem, launches,
-                       f.prm.n_units, p->num_sm, f_grid, 1 /* filter kind: direct */, 0};
+                       fft ? 16 : 2 * f.r, fft ? p->fft.threads : f.threads, fft ? 0 : f.prm.n_sb, fft ? p->fft.smem : f.smem, launches,
+                       fft ? 1 : f.prm.n_units, p->num_sm, (int)filter_ctas(p), p->filter_kind, fft ? 1 << p->fft.p : 0};
     if (out) for (int i = 0; i < n && i < 19; ++i) out[i] = v[i];
     return 19;
 }

@@ -29,6 +29,10 @@ def main() -> int:
     ap.add_argument("--dtype", default="f32", choices=["f32", "f64"])
     ap.add_argument("--reps", type=int, default=20)
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=INT")
+    ap.add_argument("--l2", default="flush", choices=["flush", "rotate", "warm"],
+                    help="flush: 256 MiB memset before every repetition (everything cold, code and tables included); "
+                         "rotate: every repetition reads another of 192 sinogram copies (> L2: inputs cold, code and tables warm); "
+                         "warm: same buffers every time")
     ap.add_argument("--dump", default=None, metavar="FILE.npy", help="also save the raw marks [CTA][8] (ns) of the last repetition")
     args = ap.parse_args()
     cfg = I.CONFIGS[args.config]
@@ -38,20 +42,24 @@ def main() -> int:
     img = torch.empty((B, cfg.image_n, cfg.image_n), dtype=tdt, device="cuda")
     options = {kv.split("=")[0]: int(kv.split("=")[1]) for kv in args.opt}
     plan = fbp.Plan(list(I.config_angles(args.config)), cfg.n_det, cfg.image_n, dtype=args.dtype, max_batch=B, options=options)
-    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda") if args.l2 == "flush" else None
+    n_pool = 192 if args.l2 == "rotate" else 1
+    pool = [sino] + [sino.clone() for _ in range(n_pool - 1)]
+    imgs = [img] + [torch.empty_like(img) for _ in range(n_pool - 1)]
     stream = torch.cuda.current_stream()
-    for _ in range(3):
-        fbp.fbp_reconstruct(plan.handle, sino, img, B, stream)
+    for i in range(3):
+        fbp.fbp_reconstruct(plan.handle, pool[i % n_pool], imgs[i % n_pool], B, stream)
     torch.cuda.synchronize()
     info = plan.info()
     n_f, n_b = info["filter_ctas"], info["bp_ctas_per_slice"] * B
     marks = torch.zeros(8 * (n_f + n_b), dtype=torch.int64, device="cuda")
     fbp.fbp_set_trace(plan.handle, marks, marks.numel())
     rows = []
-    for _ in range(args.reps):
-        flush.zero_()
+    for rep in range(args.reps):
+        if flush is not None:
+            flush.zero_()
         marks.zero_()
-        fbp.fbp_reconstruct(plan.handle, sino, img, B, stream)
+        fbp.fbp_reconstruct(plan.handle, pool[(rep + 3) % n_pool], imgs[(rep + 3) % n_pool], B, stream)
         torch.cuda.synchronize()
         m = marks.cpu().numpy().reshape(-1, 8).astype(np.float64)
         t0 = m[:n_f, 0].min()
@@ -65,7 +73,7 @@ def main() -> int:
     med = np.median(np.array(rows), axis=0)
     print("config %d %s, batch %d, options %s: %d filter CTAs x %d threads (%d units/row), %d back-projection CTAs x %d threads"
           % (args.config, args.dtype, B, options, n_f, info["filter_threads"], info["filter_units_per_row"], n_b, info["bp_threads"]))
-    print("microseconds after the first filter CTA started (median over %d flushed repetitions of min / median / max over CTAs)" % args.reps)
+    print("microseconds after the first filter CTA started (median over %d repetitions, L2 mode '%s', of min / median / max over CTAs)" % (args.reps, args.l2))
     k = 0
     for kern, slots in (("filter", FILTER_SLOTS), ("back-projection", BP_SLOTS)):
         for s in slots:

@@ -115,17 +115,19 @@ WINDOW_CASES = [  # (N, K, D, d, batch)
 ]
 
 
+@pytest.mark.parametrize("kind", [pytest.param(2, id="fft"), pytest.param(1, id="direct")])
 @pytest.mark.parametrize("dt", ["f32", "f64"])
 @pytest.mark.parametrize("window", ["shepp-logan", "cosine", "hamming", "hann"])
 @pytest.mark.parametrize("case", WINDOW_CASES)
-def test_windowed_filter_and_reconstruction_match_oracle(fbp, oracle, case, window, dt):
+def test_windowed_filter_and_reconstruction_match_oracle(fbp, oracle, case, window, dt, kind):
     import torch
     n, k, dd, d, b = case
     ang = I.uniform_angles(k)
     sino = I.random_sinogram(21 + dd, b, k, dd).astype(_np_dtype(dt))
     ref_q = oracle.filter_sinogram_window(sino.astype(np.float64), window, d)
     ref_f = oracle.backproject(ref_q, ang, n, d)
-    with fbp.Plan(list(ang), dd, n, det_spacing=d, dtype=dt, max_batch=b) as plan:
+    with fbp.Plan(list(ang), dd, n, det_spacing=d, dtype=dt, max_batch=b, options={"filter_kind": kind}) as plan:
+        assert plan.info()["filter_kind"] == kind
         plan.set_window(window)
         ds = _dev(sino, dt)
         q = plan.filter(ds)

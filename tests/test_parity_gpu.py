@@ -54,7 +54,10 @@ def check_image(gpu, ref, dt, what=""):
 # fp32 filter error measured on B200 with the conditioned sums, as a fraction of max|Q_oracle|.
 # R1 (the n-term bound below) stays the outer bar; these figures, with 2x headroom, make a regression of the
 # conditioning visible long before R1 is reached (at config 5 R1 is only 3x above what is measured).
-RECORDED_F32_FILTER_ERR = {1: 5.0e-7, 2: 8.6e-7, 3: 1.4e-6, 4: 2.5e-6, 5: 1.8e-5}
+RECORDED_F32_FILTER_ERR = {
+    1: {1: 4.1e-7, 2: 1.6e-6, 3: 1.4e-6, 4: 2.4e-6, 5: 1.8e-5},      # direct form (mirrored units; sqrt(D/2)-term sums)
+    2: {1: 1.6e-7, 2: 1.7e-7, 3: 1.2e-7, 4: 2.1e-7, 5: 1.9e-7},      # FFT form on first differences (log N deep)
+}
 
 
 def check_filter(gpu, ref, dt, what="", p_max=None, d=1.0, recorded=None):
@@ -76,7 +79,10 @@ def check_filter(gpu, ref, dt, what="", p_max=None, d=1.0, recorded=None):
     return err / bound
 
 
-def run_case(fbp, oracle, sino64, angles, n, dt, d=1.0, pix=None, what="", recorded=None):
+KINDS = [pytest.param(2, id="fft"), pytest.param(1, id="direct")]     # filter_kind of fbp_create_tuned
+
+
+def run_case(fbp, oracle, sino64, angles, n, dt, d=1.0, pix=None, what="", recorded=None, options=None):
     """Full three-way check of one geometry: filter, back-projection, reconstruct."""
     torch = _torch()
     sino64 = np.asarray(sino64, dtype=np.float64)
@@ -85,8 +91,11 @@ def run_case(fbp, oracle, sino64, angles, n, dt, d=1.0, pix=None, what="", recor
     b, k, dd = sino64.shape
     sino_in = sino64.astype(_np_dtype(dt))          # rounded once
     sino_ref = sino_in.astype(np.float64)
-    plan = fbp.Plan(list(angles), dd, n, det_spacing=d, pixel_size=0.0 if pix is None else pix, dtype=dt, max_batch=b)
+    plan = fbp.Plan(list(angles), dd, n, det_spacing=d, pixel_size=0.0 if pix is None else pix, dtype=dt, max_batch=b,
+                    options=options)
     try:
+        if options and "filter_kind" in options:
+            assert plan.info()["filter_kind"] == options["filter_kind"]
         ds = _to_dev(sino_in, dt)
         q_gpu = plan.filter(ds)
         q_ref = oracle.filter_sinogram(sino_ref, d)
@@ -109,11 +118,12 @@ def run_case(fbp, oracle, sino64, angles, n, dt, d=1.0, pix=None, what="", recor
         plan.close()
 
 
+@pytest.mark.parametrize("kind", KINDS)
 @pytest.mark.parametrize("cfg_id,dt", [(1, "f32"), (2, "f32"), (3, "f32"), (3, "f64"), (1, "f64")])
-def test_configs_full_images(fbp, oracle, cfg_id, dt):
+def test_configs_full_images(fbp, oracle, cfg_id, dt, kind):
     cfg = I.CONFIGS[cfg_id]
-    run_case(fbp, oracle, I.config_sinogram(cfg_id), I.config_angles(cfg_id), cfg.image_n, dt, what=cfg.name,
-             recorded=RECORDED_F32_FILTER_ERR[cfg_id])
+    run_case(fbp, oracle, I.config_sinogram(cfg_id), I.config_angles(cfg_id), cfg.image_n, dt, what="%s kind %d" % (cfg.name, kind),
+             recorded=RECORDED_F32_FILTER_ERR[kind][cfg_id], options={"filter_kind": kind})
 
 
 ODD_CASES = [
@@ -129,9 +139,10 @@ ODD_CASES = [
 ]
 
 
+@pytest.mark.parametrize("fkind", KINDS)
 @pytest.mark.parametrize("dt", ["f32", "f64"])
 @pytest.mark.parametrize("case", ODD_CASES)
-def test_odd_shapes_random_sinograms(fbp, oracle, case, dt):
+def test_odd_shapes_random_sinograms(fbp, oracle, case, dt, fkind):
     n, k, dd, d, pix, kind = case
     rng = np.random.default_rng(1000 + n + k)
     if kind == "uniform":
@@ -141,7 +152,7 @@ def test_odd_shapes_random_sinograms(fbp, oracle, case, dt):
     else:
         ang = np.sort(rng.uniform(-1.0, 4.0, size=k))
     sino = I.random_sinogram(77 + n, 3, k, dd)
-    run_case(fbp, oracle, sino, ang, n, dt, d, pix, what="odd%s" % (case,))
+    run_case(fbp, oracle, sino, ang, n, dt, d, pix, what="odd%s filter kind %d" % (case, fkind), options={"filter_kind": fkind})
 
 
 def _sample_pixels(n, count, seed):
@@ -156,7 +167,7 @@ def _sample_pixels(n, count, seed):
 
 
 @pytest.mark.parametrize("dt", ["f32", "f64"])
-def test_cfg5_full_image(fbp, oracle, dt):
+def test_cfg5_full_image(fbp, oracle, dt, kind=2):
     """2048^2 x 1800 x 2897 in the launch configuration bench.py uses: every filter row and EVERY pixel against the
     oracle (the oracle filters and back-projects the whole slice itself; nothing the CUDA path produced is ever an
     oracle input); DR over the full image.  This is the launch that uses the 32x32-tile back-projector."""
@@ -165,17 +176,21 @@ def test_cfg5_full_image(fbp, oracle, dt):
     sino_in = I.config_slice(5).astype(_np_dtype(dt))
     sino_ref = sino_in.astype(np.float64)
     plan = fbp.Plan(list(ang), cfg.n_det, cfg.image_n, dtype=dt, max_batch=1)
+    direct = fbp.Plan(list(ang), cfg.n_det, cfg.image_n, dtype=dt, max_batch=1, options={"filter_kind": 1})
     try:
-        assert plan.info()["bp_tile_h"] == 32
+        assert plan.info()["bp_tile_h"] == 32 and plan.info()["filter_kind"] == 2 and direct.info()["filter_kind"] == 1
         ds = _to_dev(sino_in, dt)
         q_gpu = plan.filter(ds).cpu().numpy()
         f_gpu = plan.reconstruct(ds).cpu().numpy()
+        q_direct = direct.filter(ds).cpu().numpy()
         q_ref = oracle.filter_sinogram(sino_ref)
-        check_filter(q_gpu, q_ref, dt, "cfg5 all rows", np.abs(sino_ref).max(), recorded=RECORDED_F32_FILTER_ERR[5])
+        check_filter(q_gpu, q_ref, dt, "cfg5 all rows fft", np.abs(sino_ref).max(), recorded=RECORDED_F32_FILTER_ERR[2][5])
+        check_filter(q_direct, q_ref, dt, "cfg5 all rows direct", np.abs(sino_ref).max(), recorded=RECORDED_F32_FILTER_ERR[1][5])
         f_ref = oracle.backproject(q_ref, ang, cfg.image_n)
         check_image(f_gpu, f_ref, dt, "cfg5 full image")
     finally:
         plan.close()
+        direct.close()
 
 
 def test_cfg4_batch_every_slice(fbp, oracle):
@@ -197,7 +212,7 @@ def test_cfg4_batch_every_slice(fbp, oracle):
             for i in range(8):
                 s = s0 + i
                 check_filter(q_gpu[s], q_ref[i], "f32", "cfg4 s%d" % s, np.abs(sino_in[s]).max(),
-                             recorded=RECORDED_F32_FILTER_ERR[4])
+                             recorded=RECORDED_F32_FILTER_ERR[plan.info()["filter_kind"]][4])
                 check_image(f_gpu[s], f_ref[i], "f32", "cfg4 s%d" % s)
     finally:
         plan.close()
@@ -320,14 +335,14 @@ def test_batch_pipeline_is_bit_identical_to_sequential(fbp, oracle, dt, group):
 @pytest.mark.parametrize("opts", [{"filter_sb": 1}, {"filter_sb": 3}, {"filter_sb": 8}, {"filter_r": 10}, {"filter_r": 14},
                                   {"pdl": 0}])
 def test_filter_decompositions_match_oracle(fbp, oracle, dt, opts):
-    """The row filter cuts a row into mirrored units of one warp-width (fbp_filter3.cuh): other group sizes R and other
+    """The direct-form row filter cuts a row into mirrored units of one warp-width (fbp_filter3.cuh): other group sizes R and other
     numbers of input slices must meet the same tolerances, on rows of 1, 2 and several units, and launching without
     programmatic dependent launch must not change a byte."""
     for n, k, dd, d in ((45, 9, 70, 0.5), (96, 7, 501, 1.0), (64, 5, 1203, 1.0)):
         sino = I.random_sinogram(31 + dd, 2, k, dd)
         ang = I.uniform_angles(k)
         sino_in = sino.astype(_np_dtype(dt))
-        with fbp.Plan(list(ang), dd, n, det_spacing=d, dtype=dt, max_batch=2, options=opts) as plan:
+        with fbp.Plan(list(ang), dd, n, det_spacing=d, dtype=dt, max_batch=2, options=dict(opts, filter_kind=1)) as plan:
             ds = _to_dev(sino_in, dt)
             q = plan.filter(ds)
             f = plan.reconstruct(ds)
@@ -338,7 +353,7 @@ def test_filter_decompositions_match_oracle(fbp, oracle, dt, opts):
         check_filter(q.cpu().numpy(), q_ref, dt, "units %s D=%d" % (opts, dd), np.abs(sino_in).max(), d)
         check_image(f.cpu().numpy(), oracle.reconstruct(sino_in.astype(np.float64), ang, n, d), dt, "units %s D=%d" % (opts, dd))
         if "pdl" in opts:
-            with fbp.Plan(list(ang), dd, n, det_spacing=d, dtype=dt, max_batch=2) as plain:
+            with fbp.Plan(list(ang), dd, n, det_spacing=d, dtype=dt, max_batch=2, options={"filter_kind": 1}) as plain:
                 assert _torch().equal(plain.reconstruct(ds), f)
 
 
