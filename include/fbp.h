@@ -242,8 +242,9 @@ int fbp_plan_info(const fbp_plan *plan, int *out, int n);
  *                            3 row reduced, 4 last unit stored (1-3: the CTA's first unit only)
  *   back-projector CTA c  -> d_marks[8 (F + c) + s],  F = plan_info[16],  s = 0 CTA resident, 1 past the grid
  *                            dependency, 2 first chunk landed, 3 main loop done, 4 pixels stored
- * A kernel whose records would not fit in `capacity` is not traced.  One predicated store per mark: the timed
- * kernels are the product kernels, not an instrumented build.  Not used by the batch pipeline's side streams.
+ * A kernel whose records would not fit in `capacity` is not traced.  The filters carry the marks as predicated
+ * stores; the back-projector runs a second instantiation of the same source with the marks compiled in (under its
+ * register cap even predicated-off marks cost the main loop).  Not used by the batch pipeline's side streams.
  */
 fbp_status fbp_set_trace(fbp_plan *plan, unsigned long long *d_marks, long long capacity);
 

@@ -21,4 +21,7 @@ from .oracle import (  # noqa: F401
     backproject_weighted,
     metrics,
     interpolate_stack,
+    fdk_weight,
+    fdk_backproject,
+    fdk_reconstruct,
 )

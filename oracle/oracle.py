@@ -15,6 +15,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "fbp_oracle.c")
 _SRC_EXT = os.path.join(_HERE, "fbp_oracle_ext.c")
+_SRC_FDK = os.path.join(_HERE, "fbp_oracle_fdk.c")
 _LIB = os.path.join(_HERE, "libfbp_oracle.so")
 _lock = threading.Lock()
 _lib = None
@@ -27,10 +28,10 @@ def build(force: bool = False) -> str:
     """Compile the oracle if the shared object is missing or older than its source."""
     with _lock:
         stale = (force or not os.path.exists(_LIB)
-                 or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_EXT)))
+                 or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_EXT), os.path.getmtime(_SRC_FDK)))
         if stale:
             tmp = _LIB + ".tmp.%d" % os.getpid()
-            cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-o", tmp, _SRC, _SRC_EXT, "-lm"]
+            cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-o", tmp, _SRC, _SRC_EXT, _SRC_FDK, "-lm"]
             subprocess.run(cmd, check=True)
             os.replace(tmp, _LIB)
     return _LIB
@@ -70,6 +71,13 @@ def _load():
         lib.fbp_oracle_metrics.restype = None
         lib.fbp_oracle_interpolate_stack.argtypes = [_dp, ctypes.c_int, _dp, ctypes.c_int, ctypes.c_long]
         lib.fbp_oracle_interpolate_stack.restype = None
+        lib.fbp_oracle_fdk_weight.argtypes = [_dp, _dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double,
+                                              ctypes.c_double, ctypes.c_double]
+        lib.fbp_oracle_fdk_weight.restype = None
+        lib.fbp_oracle_fdk_backproject.argtypes = [_dp, _dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp, ctypes.c_double,
+                                                   ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_double,
+                                                   ctypes.c_int, ctypes.c_double, ctypes.c_int]
+        lib.fbp_oracle_fdk_backproject.restype = None
         for fn in ("fbp_oracle_taps", "fbp_oracle_filter", "fbp_oracle_backproject",
                    "fbp_oracle_backproject_pixels", "fbp_oracle_filter_rows",
                    "fbp_oracle_forward_scatter", "fbp_oracle_reconstruct"):
@@ -247,3 +255,39 @@ def interpolate_stack(stack, n_out: int) -> np.ndarray:
     out = np.empty((int(n_out),) + a.shape[1:], dtype=np.float64)
     lib.fbp_oracle_interpolate_stack(_p(a), a.shape[0], _p(out), int(n_out), a.shape[1] * a.shape[2])
     return out
+
+
+# ---- cone-beam FDK (fbp_oracle_fdk.c) -----------------------------------------------------------
+def fdk_weight(proj, d_a: float, d_b: float, sad: float) -> np.ndarray:
+    """C3: cosine pre-weight sad / sqrt(sad^2 + a^2 + b^2) of projections [K][n_b][n_a]."""
+    lib = _load()
+    p = _f64(proj)
+    assert p.ndim == 3
+    out = np.empty_like(p)
+    lib.fbp_oracle_fdk_weight(_p(p), _p(out), p.shape[0], p.shape[1], p.shape[2], float(d_a), float(d_b), float(sad))
+    return out
+
+
+def fdk_backproject(filtered, angles, sad: float, image_n: int, n_z: int, d_a: float = 1.0, d_b: float = 1.0,
+                    pixel_size: float | None = None, voxel_z: float | None = None, threads: int = 0) -> np.ndarray:
+    """C5: volume [n_z][N][N] from filtered, weighted projections [K][n_b][n_a]."""
+    lib = _load()
+    q = _f64(filtered)
+    ang = _f64(angles)
+    assert q.ndim == 3 and ang.shape == (q.shape[0],)
+    pix = float(d_a if pixel_size is None else pixel_size)
+    vz = float(pix if voxel_z is None else voxel_z)
+    f = np.empty((int(n_z), int(image_n), int(image_n)), dtype=np.float64)
+    lib.fbp_oracle_fdk_backproject(_p(q), _p(f), q.shape[0], q.shape[1], q.shape[2], _p(ang), float(d_a), float(d_b),
+                                   float(sad), int(image_n), pix, int(n_z), vz, int(threads))
+    return f
+
+
+def fdk_reconstruct(proj, angles, sad: float, image_n: int, n_z: int, d_a: float = 1.0, d_b: float = 1.0,
+                    pixel_size: float | None = None, voxel_z: float | None = None, threads: int = 0) -> np.ndarray:
+    """FDK end to end: pre-weight (C3), Ram-Lak row filter (C4 = O2 of fbp_oracle.c on every detector row),
+    weighted cone-beam back-projection (C5)."""
+    w = fdk_weight(proj, d_a, d_b, sad)
+    k, nb, na = w.shape
+    q = filter_sinogram(w.reshape(k * nb, na), d_a, threads).reshape(k, nb, na)
+    return fdk_backproject(q, angles, sad, image_n, n_z, d_a, d_b, pixel_size, voxel_z, threads)

@@ -514,7 +514,8 @@ cudaError_t launch_fft_p(fbp_plan* p, const void* sino, void* filt, void* ent, i
         if (per_sm < 1) return cudaErrorLaunchOutOfResources;
         c.grid_cap = per_sm * p->num_sm;
     }
-    fbp::FftParams f{batch, p->K, p->D, (p->K + 1) / 2, p->bp.ent_pitch, p->bp.ent_guard, c.buf_bytes, nullptr};
+    fbp::FftParams f{batch, p->K, p->D, (p->K + 1) / 2, p->bp.ent_pitch, p->bp.ent_guard, c.buf_bytes,
+                     ent ? p->d_cs2 : nullptr, (int)(sizeof(double2) * (size_t)p->K), nullptr};
     const long long work = (long long)batch * f.pairs_per_slice;
     const int grid = (int)std::min<long long>(work, c.grid_cap);
     if (p->d_trace && 8LL * grid <= p->trace_cap) f.trace = p->d_trace;
@@ -582,10 +583,10 @@ long long filter_ctas(const fbp_plan* p)
     return f.grid_cap > 0 ? std::min<long long>((long long)p->max_batch * p->K * f.prm.n_units, f.grid_cap) : 0;
 }
 
-template <typename T, int R, int WY, int WA>
-cudaError_t launch_bp_v(fbp_plan* p, void* image, int batch, cudaStream_t st, int slice0)
+template <typename T, int R, int WY, int WA, bool TRACE>
+cudaError_t launch_bp_t(fbp_plan* p, void* image, int batch, cudaStream_t st, int slice0)
 {
-    auto kern = fbp::backproject_kernel<T, R, WY, WA>;
+    auto kern = fbp::backproject_kernel<T, R, WY, WA, TRACE>;
     static bool smem_open[kMaxDevices] = {};     // per instantiation and device
     if (cudaError_t e = allow_max_smem(kern, smem_open, p->device); e != cudaSuccess) return e;
     // programmatic dependent launch: the CTAs may become resident and run their prologue while the
@@ -614,6 +615,13 @@ cudaError_t launch_bp_v(fbp_plan* p, void* image, int batch, cudaStream_t st, in
     }
     return cudaLaunchKernelEx(&cfg, kern, ent, static_cast<T*>(image),
                               static_cast<const double2*>(p->d_cs2), static_cast<T*>(p->d_part), p->d_tickets, prm);
+}
+
+template <typename T, int R, int WY, int WA>
+cudaError_t launch_bp_v(fbp_plan* p, void* image, int batch, cudaStream_t st, int slice0)
+{
+    return p->d_trace ? launch_bp_t<T, R, WY, WA, true>(p, image, batch, st, slice0)
+                      : launch_bp_t<T, R, WY, WA, false>(p, image, batch, st, slice0);
 }
 
 // back-projection of the plan's entry buffer into `image`

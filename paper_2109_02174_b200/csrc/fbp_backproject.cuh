@@ -118,6 +118,8 @@ template <> struct PairAcc<double> {
 // cs2: [K] pairs (cos*pix/d, sin*pix/d) in fp64.  E: 16-byte entry units [batch][K][planes][pitch].
 // Grid (tiles, S, batch).  image: [batch][N][N], fully written, scaled by pi/K.
 // part: scratch [S][batch][N][N] and tickets: [batch][tiles] zero-initialised counters (S > 1 only).
+// TRACE: the instantiation launched while fbp_set_trace is on (the marks are compiled out of the other one: under its
+// 64-register cap even predicated-off stores cost the main loop 1.5 us at config 3).
 // Registers per thread the occupancy bound aims at.  fp32: 64 for the small-tile variants (6 CTAs of 160 threads per SM),
 // 72 for the 32x32 tile (R = 8, WY = 4: at 64 the 16 packed accumulators spill 48 bytes; measured 1.84 -> 1.78 ms at
 // config 5, 2.88 -> 2.84 ms at config 4).  fp64: 96, and 112 for the 32x32 tile (3.60 -> 3.52 ms at config 5).
@@ -132,7 +134,7 @@ template <> struct PairAcc<double> {
 #endif
 constexpr int kBpStages = FBP_BP_STAGES;
 
-template <typename T, int R, int WY, int WA>
+template <typename T, int R, int WY, int WA, bool TRACE>
 __global__ void __launch_bounds__(32 * (WY * WA + 1), 65536 / (FBP_BP_REGCAP * 32 * (WY * WA + 1)))
 backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const double2* __restrict__ cs2,
                    T* __restrict__ part, int* __restrict__ tickets, BpParams prm)
@@ -153,7 +155,7 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned cta_id = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
-    trace_mark(prm.trace, cta_id, 0);                          // CTA resident
+    if (TRACE) trace_mark(prm.trace, cta_id, 0);               // CTA resident
     const bool producer = warp == NW;
     const int wy = warp % WY, wa = producer ? WA : warp / WY;
     const int tile = blockIdx.x;
@@ -180,7 +182,7 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
     // E.  Every thread blocks here (consumers would otherwise spin on their mbarriers and take issue
     // slots from that kernel); a no-op when launched without the attribute.
     asm volatile("griddepcontrol.wait;" ::: "memory");
-    trace_mark(prm.trace, cta_id, 1);                          // past the grid dependency
+    if (TRACE) trace_mark(prm.trace, cta_id, 1);               // past the grid dependency
 
     PairAcc<T> acc[R];
 #pragma unroll
@@ -235,7 +237,7 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
             const int st = k % NS;
             const int na = min(prm.chunk, a_end - (a_begin + k * prm.chunk));
             mbar_wait(bar_full + 8u * st, (unsigned)((k / NS) & 1));  // chunk k has landed
-            if (k == 0) trace_mark(prm.trace, cta_id, 2);      // first chunk landed (thread 0 is a consumer)
+            if (TRACE && k == 0) trace_mark(prm.trace, cta_id, 2);   // first chunk landed (thread 0 is a consumer)
             const AngleRec<T>* rk = rec + st * prm.chunk;
             const unsigned segk = seg + st * stage_stride - Magic<T>::kBits * 16u;  // bits(M) folded in
 #pragma unroll 2
@@ -256,7 +258,7 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
         }
     }
 
-    trace_mark(prm.trace, cta_id, 3);                          // main loop done
+    if (TRACE) trace_mark(prm.trace, cta_id, 3);               // main loop done
     // ---- in-CTA reduction over the WA angle groups, fixed order g = 0..WA-1 ----
     T va[R], vb[R];
 #pragma unroll
@@ -301,7 +303,7 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
             if (ok_a(r)) img[base_a + (long long)r * N] = va[r] * sc;
             if (ok_b(r)) img[base_b - (long long)r * N] = vb[r] * sc;
         }
-        trace_mark(prm.trace, cta_id, 4);                      // pixels stored
+        if (TRACE) trace_mark(prm.trace, cta_id, 4);           // pixels stored
         return;
     }
 

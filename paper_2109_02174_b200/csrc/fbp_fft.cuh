@@ -40,6 +40,8 @@ struct FftParams {
     int pairs_per_slice;             // ceil(K / 2)
     int ent_pitch, ent_guard;
     int buf_bytes;                   // bytes of the transform / row buffer region (a multiple of 16)
+    const void* warm;                // a table of the NEXT kernel (the back-projector's cos/sin) to start into L2, or NULL
+    int warm_bytes;
     unsigned long long* trace;
 };
 
@@ -203,6 +205,11 @@ fft_filter_kernel(const T* __restrict__ Pin, T* __restrict__ Q, uint4* __restric
 
     pdl_launch_dependents();
     trace_mark(prm.trace, blockIdx.x, 0);
+    // the back-projector's first instruction after its grid dependency is a read of its cos/sin table, which nothing
+    // has touched since the caller's last use of the plan: one CTA starts it on its way into L2 now
+    if (blockIdx.x == 0 && prm.warm != nullptr)
+        for (int i = tid * 128; i < prm.warm_bytes; i += nthr * 128)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(static_cast<const char*>(prm.warm) + i));
     if (TSMEM) {
         // one bulk copy brings the whole table in while the first pass reads the rows
         const unsigned bar = smem_u32(fft_smem_raw);

@@ -243,3 +243,32 @@ def random_sinogram(seed: int, batch: int, n_angles: int, n_det: int) -> np.ndar
 
 def sha256(a: np.ndarray) -> str:
     return hashlib.sha256(np.ascontiguousarray(a).tobytes()).hexdigest()
+
+
+# ---------------------------------------------------------------------------------------
+# Cone-beam inputs for the FDK row: analytic line integrals of balls.
+# Geometry as include/fbp.h "fbp_fdk_reconstruct": source at -sad * e_s(beta), e_s = (-sin, cos, 0); flat virtual
+# detector through the rotation axis spanned by e_a = (cos, sin, 0) and e_z, centred, spacings d_a and d_b.
+# ---------------------------------------------------------------------------------------
+
+def ball_cone_projections(balls, angles, sad, n_a, n_b, d_a=1.0, d_b=1.0) -> np.ndarray:
+    """P[K][n_b][n_a] (fp64): sum over balls (rho, radius, x0, y0, z0) of rho * chord length of the ray from the
+    source through the detector point (a_j, b_i); chord = 2 sqrt(radius^2 - dist^2), dist = distance from the
+    ball's centre to the ray (closed form; point-sampled at the detector pixel centres)."""
+    balls = np.atleast_2d(np.asarray(balls, dtype=np.float64))
+    angles = np.asarray(angles, dtype=np.float64)
+    a = detector_coords(n_a, d_a)[None, None, :]
+    b = detector_coords(n_b, d_b)[None, :, None]
+    cb, sb = np.cos(angles)[:, None, None], np.sin(angles)[:, None, None]
+    # source S = -sad * e_s, detector point D = a e_a + b e_z, direction v = D - S
+    sx, sy = sad * sb, -sad * cb
+    vx, vy, vz = a * cb - sx, a * sb - sy, b + 0.0 * a
+    vn = np.sqrt(vx * vx + vy * vy + vz * vz)
+    vx, vy, vz = vx / vn, vy / vn, vz / vn
+    out = np.zeros((angles.size, n_b, n_a), dtype=np.float64)
+    for rho, rad, x0, y0, z0 in balls:
+        wx, wy, wz = x0 - sx, y0 - sy, z0 + 0.0 * sx          # centre - source
+        along = wx * vx + wy * vy + wz * vz
+        dist2 = wx * wx + wy * wy + wz * wz - along * along
+        out += rho * 2.0 * np.sqrt(np.maximum(rad * rad - dist2, 0.0))
+    return out
