@@ -352,7 +352,18 @@ def measure(args, dtype, world, rank, local, dist):
         for _ in range(3):
             pfn()
         p_ms = timed_loop(pfn, 10) / 10
-        extras = {"project_ms": p_ms, "project_slices": pb,
+        # fbp_fdk_reconstruct: cone-beam FDK of a 64-slice volume on the config's x-y grid from n_det x 97 projections
+        # (pre-weight + row filter + weighted bilinear back-projection); voxel-angle updates per second of the whole call
+        n_rows, n_z, sad = 97, 64, 2.0 * N
+        d_cone = torch.empty((K, n_rows, D), dtype=tdt, device="cuda").normal_()
+        d_vol = torch.empty((n_z, N, N), dtype=tdt, device="cuda")
+        kfn = lambda: fbp.fbp_fdk_reconstruct(plan.handle, d_cone, d_vol, n_rows, 1.0, sad, n_z, 1.0, stream)  # noqa: E731
+        for _ in range(2):
+            kfn()
+        k_ms = timed_loop(kfn, 5) / 5
+        extras = {"fdk_ms": k_ms, "fdk_volume": [n_z, N, N], "fdk_detector_rows": n_rows,
+                  "fdk_gupdates_per_s": float(n_z) * N * N * K / (k_ms * 1e-3) / 1e9,
+                  "project_ms": p_ms, "project_slices": pb,
                   "project_gupdates_per_s": float(pb) * N * N * K / (p_ms * 1e-3) / 1e9,
                   "stack_interp_ms": i_ms, "stack_interp_gbs": i_bytes / (i_ms * 1e-3) / 1e9, "stack_interp_bytes": i_bytes,
                   "stack_interp_slices_out": n_out,

@@ -197,6 +197,28 @@ fbp_status fbp_set_angle_weights(fbp_plan *plan, const double *h_weights);
 fbp_status fbp_project(fbp_plan *plan, const void *d_image, void *d_sino, int batch, void *cuda_stream);
 
 /*
+ * fbp_fdk_reconstruct -- cone-beam reconstruction by the algorithm of Feldkamp, Davis and Kress, the continuation the
+ * paper announces (ref [20]: it "uses the filtered backprojection algorithm in the reconstruction of
+ * three-dimensional images obtained by projections of a cone beam").  The paper gives no
+ * formula; this is the textbook algorithm (Kak & Slaney ch. 3.6, ref [8]) in the plan's 2-D conventions.  Readings
+ * (DESIGN.md "FDK"): circular source orbit of radius `sad` about the z axis in the plane z = 0, source at
+ * -sad * e_s(beta), e_s = (-sin beta, cos beta, 0); flat VIRTUAL detector through the axis spanned by
+ * e_a = (cos beta, sin beta, 0) (columns: the plan's n_det bins of det_spacing, centred) and e_z (n_rows rows of
+ * row_spacing, centred); angles = the plan's (meant to cover [0, 2 pi) uniformly); x, y grid = the plan's image grid,
+ * z_k = (k - (n_z-1)/2) voxel_z.
+ *   1. p'[m][i][j] = p[m][i][j] * sad / sqrt(sad^2 + a_j^2 + b_i^2)
+ *   2. Q[m][i][:]  = the plan's row filter applied to every detector row (fbp_filter's operation; fbp_set_window applies)
+ *   3. f[k][r][c]  = (pi/K) sum_m (sad/U)^2 bilinear(Q[m]; sad t/(U d_a) + (n_det-1)/2, sad z_k/(U d_b) + (n_rows-1)/2),
+ *                    t = x cos + y sin,  U = sad - x sin + y cos,  zero outside the detector.
+ * d_proj [K][n_rows][n_det] in, d_volume [n_z][N][N] out (DEVICE, plan dtype, 16-byte aligned).  sad must exceed the
+ * image's half-diagonal (FBP_EINVAL otherwise).  The first call (and any call with more rows than before) allocates
+ * plan-owned scratch (synchronous); later calls only enqueue.  One owner thread per voxel, fixed order: deterministic.
+ * Angle weights do not apply.
+ */
+fbp_status fbp_fdk_reconstruct(fbp_plan *plan, const void *d_proj, void *d_volume, int n_rows, double row_spacing,
+                               double sad, int n_z, double voxel_z, void *cuda_stream);
+
+/*
  * fbp_interpolate_stack -- a volume from a stack of reconstructed slices (3-D images
  * "through the interpolation of a stack of 2D images"; the paper names no rule, LINEAR is the reading
  * taken, R4).  d_stack [n_in][N][N] in, d_out [n_out][N][N] out (DEVICE, plan dtype, may not

@@ -10,7 +10,7 @@ from .binding import (  # noqa: F401
     EXPORTS, FBP_F32, FBP_F64, FBP_OK, FBP_EINVAL, FBP_ENOMEM, FBP_ECUDA, FBP_EUNSUPPORTED,
     FbpError, load_library,
     fbp_create, fbp_create_tuned, OPTIONS, fbp_filter, fbp_backproject, fbp_reconstruct, fbp_reconstruct_host,
-    fbp_destroy, fbp_last_error, fbp_plan_info, fbp_set_profiling, fbp_get_kernel_ms, fbp_set_trace, fbp_metrics, fbp_set_window, fbp_set_angle_weights, WINDOWS, fbp_interpolate_stack, fbp_project,
+    fbp_destroy, fbp_last_error, fbp_plan_info, fbp_set_profiling, fbp_get_kernel_ms, fbp_set_trace, fbp_metrics, fbp_set_window, fbp_set_angle_weights, WINDOWS, fbp_interpolate_stack, fbp_project, fbp_fdk_reconstruct,
 )
 from .build import build  # noqa: F401
 
@@ -107,6 +107,22 @@ class Plan:
               or tuple(out.shape) != (int(n_out), self.image_n, self.image_n)):
             raise ValueError("out must be a contiguous CUDA tensor [n_out][N][N] of the plan dtype")
         fbp_interpolate_stack(self.handle, stack, stack.shape[0], out, n_out, stream)
+        return out
+
+    def fdk_reconstruct(self, proj, sad, n_z, row_spacing=1.0, voxel_z=None, out=None, stream=None):
+        """Cone-beam FDK: projections [K][n_rows][n_det] -> volume [n_z][N][N] (include/fbp.h, fbp_fdk_reconstruct)."""
+        import torch
+        if (proj.dtype != self.torch_dtype or not proj.is_cuda or not proj.is_contiguous() or proj.dim() != 3
+                or proj.shape[0] != self.n_angles or proj.shape[2] != self.n_det):
+            raise ValueError("expected a contiguous CUDA tensor [K][n_rows][n_det] of the plan dtype")
+        shape = (int(n_z), self.image_n, self.image_n)
+        if out is None:
+            out = torch.empty(shape, dtype=self.torch_dtype, device=proj.device)
+        elif (out.dtype != self.torch_dtype or not out.is_cuda or not out.is_contiguous() or tuple(out.shape) != shape
+              or out.device != proj.device):
+            raise ValueError("out must be a contiguous CUDA tensor [n_z][N][N] of the plan dtype")
+        fbp_fdk_reconstruct(self.handle, proj, out, proj.shape[1], row_spacing, sad, n_z,
+                            row_spacing if voxel_z is None else voxel_z, stream)
         return out
 
     def set_window(self, window):

@@ -18,7 +18,7 @@ STATUS_NAMES = {0: "FBP_OK", 1: "FBP_EINVAL", 2: "FBP_ENOMEM", 3: "FBP_ECUDA", 4
 EXPORTS = (
     "fbp_create", "fbp_create_tuned", "fbp_filter", "fbp_backproject", "fbp_reconstruct", "fbp_reconstruct_host",
     "fbp_destroy", "fbp_last_error", "fbp_plan_info", "fbp_set_profiling", "fbp_get_kernel_ms",
-    "fbp_set_trace", "fbp_metrics", "fbp_set_window", "fbp_set_angle_weights", "fbp_interpolate_stack", "fbp_project",
+    "fbp_set_trace", "fbp_metrics", "fbp_set_window", "fbp_set_angle_weights", "fbp_interpolate_stack", "fbp_project", "fbp_fdk_reconstruct",
 )
 
 PLAN_INFO_FIELDS = (
@@ -73,6 +73,8 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     lib.fbp_set_angle_weights.restype = ci
     lib.fbp_interpolate_stack.argtypes = [vp, vp, ci, vp, ci, vp]
     lib.fbp_interpolate_stack.restype = ci
+    lib.fbp_fdk_reconstruct.argtypes = [vp, vp, vp, ci, cd, cd, ci, cd, vp]
+    lib.fbp_fdk_reconstruct.restype = ci
     lib.fbp_destroy.argtypes = [vp]
     lib.fbp_destroy.restype = None
     lib.fbp_last_error.argtypes = [vp]
@@ -247,3 +249,9 @@ def fbp_interpolate_stack(plan, d_stack, n_in, d_out, n_out, stream=None):
 def fbp_project(plan, d_image, d_sino, batch, stream=None):
     lib = load_library()
     _check(lib, plan, lib.fbp_project(plan, _ptr(d_image), _ptr(d_sino), int(batch), _stream_handle(stream)))
+
+
+def fbp_fdk_reconstruct(plan, d_proj, d_volume, n_rows, row_spacing, sad, n_z, voxel_z, stream=None):
+    lib = load_library()
+    _check(lib, plan, lib.fbp_fdk_reconstruct(plan, _ptr(d_proj), _ptr(d_volume), int(n_rows), float(row_spacing), float(sad),
+                                              int(n_z), float(voxel_z), _stream_handle(stream)))

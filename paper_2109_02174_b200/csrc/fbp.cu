@@ -22,6 +22,7 @@
 #include "fbp_metrics.cuh"
 #include "fbp_stack.cuh"
 #include "fbp_project.cuh"
+#include "fbp_fdk.cuh"
 
 namespace {
 
@@ -81,6 +82,8 @@ struct fbp_plan {
     int filter_kind = 1;        // 1 direct form, 2 FFT form
     int window = 0;             // fbp_set_window; 0 = Ram-Lak
     void* d_xt = nullptr;       // 2 x [max_batch][N][N + 2 pad] dtype: padded image and padded transpose for fbp_project
+    void* d_fdk = nullptr;      // 2 x [K][n_rows][n_det] dtype: weighted and filtered cone-beam projections (fbp_fdk_reconstruct)
+    size_t fdk_elems = 0;
     void* d_wrow = nullptr;     // [K] dtype: angle weight / (pi/K) (fbp_set_angle_weights); NULL = uniform
 
     double* d_mscratch = nullptr;   // fbp_metrics: [kMetricGridMax][3] CTA partials, then mid[3], ticket
@@ -473,12 +476,13 @@ cudaError_t upload_filter3_tables(fbp_plan* p, bool dense, int window)
 
 // ---- kernel launchers ---------------------------------------------------------------
 // filt and/or ent may be NULL: plain rows (fbp_filter) and/or entries (fbp_reconstruct)
+// rows: rows per slice (the plan's K, or K * n_rows for the cone-beam path, whose rows carry no entries)
 template <typename T, int R, bool DENSE>
-cudaError_t launch_filter3_r(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st)
+cudaError_t launch_filter3_r(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st, int rows)
 {
     fbp_plan::F3& c = p->f3[DENSE ? 1 : 0];
     fbp::Filter3Params f = c.prm;
-    f.n_rows = batch * p->K;
+    f.n_rows = batch * rows;
     f.trace = nullptr;
     auto kern = fbp::filter3_kernel<T, R, DENSE>;
     static bool smem_open[kMaxDevices] = {};
@@ -501,7 +505,7 @@ cudaError_t launch_filter3_r(fbp_plan* p, const void* sino, void* filt, void* en
 }
 
 template <typename T, int P, bool TSMEM>
-cudaError_t launch_fft_p(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st)
+cudaError_t launch_fft_p(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st, int rows)
 {
     fbp_plan::Fft& c = p->fft;
     auto kern = fbp::fft_filter_kernel<T, P, TSMEM>;
@@ -514,7 +518,7 @@ cudaError_t launch_fft_p(fbp_plan* p, const void* sino, void* filt, void* ent, i
         if (per_sm < 1) return cudaErrorLaunchOutOfResources;
         c.grid_cap = per_sm * p->num_sm;
     }
-    fbp::FftParams f{batch, p->K, p->D, (p->K + 1) / 2, p->bp.ent_pitch, p->bp.ent_guard, c.buf_bytes,
+    fbp::FftParams f{batch, rows, p->D, (rows + 1) / 2, p->bp.ent_pitch, p->bp.ent_guard, c.buf_bytes,
                      ent ? p->d_cs2 : nullptr, (int)(sizeof(double2) * (size_t)p->K), nullptr};
     const long long work = (long long)batch * f.pairs_per_slice;
     const int grid = (int)std::min<long long>(work, c.grid_cap);
@@ -525,40 +529,42 @@ cudaError_t launch_fft_p(fbp_plan* p, const void* sino, void* filt, void* ent, i
 }
 
 template <typename T, bool TSMEM>
-cudaError_t launch_fft_t(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st)
+cudaError_t launch_fft_t(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st, int rows)
 {
     switch (p->fft.p) {
-        case 6: return launch_fft_p<T, 6, TSMEM>(p, sino, filt, ent, batch, st);
-        case 7: return launch_fft_p<T, 7, TSMEM>(p, sino, filt, ent, batch, st);
-        case 8: return launch_fft_p<T, 8, TSMEM>(p, sino, filt, ent, batch, st);
-        case 9: return launch_fft_p<T, 9, TSMEM>(p, sino, filt, ent, batch, st);
-        case 10: return launch_fft_p<T, 10, TSMEM>(p, sino, filt, ent, batch, st);
-        case 11: return launch_fft_p<T, 11, TSMEM>(p, sino, filt, ent, batch, st);
-        case 12: return launch_fft_p<T, 12, TSMEM>(p, sino, filt, ent, batch, st);
-        default: return launch_fft_p<T, 13, TSMEM>(p, sino, filt, ent, batch, st);
+        case 6: return launch_fft_p<T, 6, TSMEM>(p, sino, filt, ent, batch, st, rows);
+        case 7: return launch_fft_p<T, 7, TSMEM>(p, sino, filt, ent, batch, st, rows);
+        case 8: return launch_fft_p<T, 8, TSMEM>(p, sino, filt, ent, batch, st, rows);
+        case 9: return launch_fft_p<T, 9, TSMEM>(p, sino, filt, ent, batch, st, rows);
+        case 10: return launch_fft_p<T, 10, TSMEM>(p, sino, filt, ent, batch, st, rows);
+        case 11: return launch_fft_p<T, 11, TSMEM>(p, sino, filt, ent, batch, st, rows);
+        case 12: return launch_fft_p<T, 12, TSMEM>(p, sino, filt, ent, batch, st, rows);
+        default: return launch_fft_p<T, 13, TSMEM>(p, sino, filt, ent, batch, st, rows);
     }
 }
 template <typename T>
-cudaError_t launch_fft(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st)
+cudaError_t launch_fft(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st, int rows)
 {
-    return p->fft.tab_smem ? launch_fft_t<T, true>(p, sino, filt, ent, batch, st) : launch_fft_t<T, false>(p, sino, filt, ent, batch, st);
+    return p->fft.tab_smem ? launch_fft_t<T, true>(p, sino, filt, ent, batch, st, rows)
+                           : launch_fft_t<T, false>(p, sino, filt, ent, batch, st, rows);
 }
 
 template <typename T>
-cudaError_t launch_filter(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st)
+cudaError_t launch_filter(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st, int rows = 0)
 {
-    if (p->filter_kind == 2) return launch_fft<T>(p, sino, filt, ent, batch, st);
+    if (rows <= 0) rows = p->K;
+    if (p->filter_kind == 2) return launch_fft<T>(p, sino, filt, ent, batch, st, rows);
     if (p->window != 0) {
         switch (p->f3[1].r) {
-            case 5: return launch_filter3_r<T, 5, true>(p, sino, filt, ent, batch, st);
-            case 7: return launch_filter3_r<T, 7, true>(p, sino, filt, ent, batch, st);
-            default: return launch_filter3_r<T, 9, true>(p, sino, filt, ent, batch, st);
+            case 5: return launch_filter3_r<T, 5, true>(p, sino, filt, ent, batch, st, rows);
+            case 7: return launch_filter3_r<T, 7, true>(p, sino, filt, ent, batch, st, rows);
+            default: return launch_filter3_r<T, 9, true>(p, sino, filt, ent, batch, st, rows);
         }
     }
     switch (p->f3[0].r) {
-        case 6: return launch_filter3_r<T, 6, false>(p, sino, filt, ent, batch, st);
-        case 10: return launch_filter3_r<T, 10, false>(p, sino, filt, ent, batch, st);
-        default: return launch_filter3_r<T, 14, false>(p, sino, filt, ent, batch, st);
+        case 6: return launch_filter3_r<T, 6, false>(p, sino, filt, ent, batch, st, rows);
+        case 10: return launch_filter3_r<T, 10, false>(p, sino, filt, ent, batch, st, rows);
+        default: return launch_filter3_r<T, 14, false>(p, sino, filt, ent, batch, st, rows);
     }
 }
 
@@ -897,7 +903,7 @@ void fbp_destroy(fbp_plan* p)
     {
         DeviceGuard guard(p->device);
         cudaFree(p->d_cs2); cudaFree(p->d_ent); cudaFree(p->d_part); cudaFree(p->d_tickets);
-        cudaFree(p->d_hsino); cudaFree(p->d_himg); cudaFree(p->d_mscratch); cudaFree(p->d_wrow); cudaFree(p->d_xt);
+        cudaFree(p->d_hsino); cudaFree(p->d_himg); cudaFree(p->d_mscratch); cudaFree(p->d_wrow); cudaFree(p->d_xt); cudaFree(p->d_fdk);
         for (int i = 0; i < 2; ++i) { cudaFree(p->f3[i].d_u); cudaFree(p->f3[i].d_rho); }
         cudaFree(p->fft.d_tab);
         for (int i = 0; i < 4; ++i) if (p->ev[i]) cudaEventDestroy(p->ev[i]);
@@ -1073,6 +1079,57 @@ fbp_status fbp_project(fbp_plan* p, const void* d_image, void* d_sino, int batch
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(p, e, "projector launch");
+    return FBP_OK;
+}
+
+fbp_status fbp_fdk_reconstruct(fbp_plan* p, const void* d_proj, void* d_volume, int n_rows, double row_spacing, double sad,
+                               int n_z, double voxel_z, void* stream)
+{
+    if (!p) return FBP_EINVAL;
+    if (!d_proj || !d_volume) return fail(p, FBP_EINVAL, "NULL device pointer");
+    if (!aligned16(d_proj) || !aligned16(d_volume)) return fail(p, FBP_EINVAL, "device pointers must be 16-byte aligned");
+    if (n_rows < 1 || n_rows > (1 << 16) || n_z < 1 || n_z > (1 << 16)) return fail(p, FBP_EINVAL, "n_rows and n_z must be in [1, 65536]");
+    if (!(row_spacing > 0.0) || !std::isfinite(row_spacing) || !(voxel_z > 0.0) || !std::isfinite(voxel_z))
+        return fail(p, FBP_EINVAL, "row_spacing and voxel_z must be finite and > 0");
+    // every voxel must lie strictly inside the source orbit: U = sad + s > 0 with |s| <= (N-1)/2 sqrt(2) pix
+    const double reach = 0.5 * (p->N - 1) * std::sqrt(2.0) * p->pix;
+    if (!std::isfinite(sad) || !(sad > reach)) return fail(p, FBP_EINVAL, "sad must be finite and exceed the half-diagonal of the image");
+    const long long rows = (long long)p->K * n_rows;
+    if (rows > 0x7fffffffLL / 2) return fail(p, FBP_EINVAL, "too many projection rows");
+    DeviceGuard guard(p->device);
+    const size_t elems = (size_t)rows * p->D;
+    if (elems > p->fdk_elems) {                      // first call (or a taller detector): synchronous, like fbp_project
+        FBP_CUDA(p, cudaDeviceSynchronize());
+        cudaFree(p->d_fdk);
+        p->d_fdk = nullptr; p->fdk_elems = 0;
+        FBP_CUDA(p, cudaMalloc(&p->d_fdk, 2 * elems * p->esize));
+        p->fdk_elems = elems;
+    }
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    void* weighted = p->d_fdk;
+    void* filtered = static_cast<char*>(p->d_fdk) + elems * p->esize;
+    const unsigned wgrid = (unsigned)((elems + 255) / 256);
+    fbp::FdkParams prm{p->K, p->D, n_rows, p->N, n_z, sad / p->d, voxel_z / row_spacing,
+                       0.5 * (p->N - 1), 0.5 * (n_z - 1), 0.5 * (p->D - 1), 0.5 * (n_rows - 1), kPi / p->K};
+    const dim3 bgrid((p->N + 31) / 32, (p->N + 3) / 4, (n_z + fbp::kFdkZT - 1) / fbp::kFdkZT), bblock(32, 4);
+    cudaError_t e;
+    if (p->dtype == FBP_F32) {
+        fbp::fdk_weight_kernel<float><<<wgrid, 256, 0, s>>>(static_cast<const float*>(d_proj), static_cast<float*>(weighted),
+                                                            (long long)elems, p->D, n_rows, p->d, row_spacing, sad);
+        e = launch_filter<float>(p, weighted, filtered, nullptr, 1, s, (int)rows);
+        if (e == cudaSuccess)
+            fbp::fdk_backproject_kernel<float><<<bgrid, bblock, 0, s>>>(static_cast<const float*>(filtered),
+                                                                        static_cast<float*>(d_volume), p->d_cs2, prm);
+    } else {
+        fbp::fdk_weight_kernel<double><<<wgrid, 256, 0, s>>>(static_cast<const double*>(d_proj), static_cast<double*>(weighted),
+                                                             (long long)elems, p->D, n_rows, p->d, row_spacing, sad);
+        e = launch_filter<double>(p, weighted, filtered, nullptr, 1, s, (int)rows);
+        if (e == cudaSuccess)
+            fbp::fdk_backproject_kernel<double><<<bgrid, bblock, 0, s>>>(static_cast<const double*>(filtered),
+                                                                         static_cast<double*>(d_volume), p->d_cs2, prm);
+    }
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(p, e, "FDK launch");
     return FBP_OK;
 }
 
