@@ -54,6 +54,8 @@ def parse_args():
                     help="reconstruction filter (SURVEY.md 8(f) row 1); the headline is ramlak")
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=INT",
                     help="launch-configuration override passed to fbp_create_tuned (A/B runs), e.g. --opt filter_kind=1")
+    ap.add_argument("--graph", action="store_true",
+                    help="also time the step replayed as ONE CUDA graph (the two launches with their programmatic edge captured once)")
     ap.add_argument("--extras", action="store_true", help="also time fbp_metrics, fbp_interpolate_stack and fbp_project")
     return ap.parse_args()
 
@@ -308,6 +310,24 @@ def measure(args, dtype, world, rank, local, dist):
     ms_step = ms_total / args.steps
     info = plan.info()
 
+    # the same step replayed as a CUDA graph (captured once on a side stream after the warm-up above)
+    graph_ms = None
+    if args.graph:
+        side = torch.cuda.Stream()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(side):
+            fbp.fbp_reconstruct(plan.handle, d_sino, d_img, B, side)
+            side.synchronize()
+            with torch.cuda.graph(g, stream=side):
+                fbp.fbp_reconstruct(plan.handle, d_sino, d_img, B, torch.cuda.current_stream())
+        want = d_img.clone()
+        step()
+        torch.cuda.synchronize()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(d_img, want), "graph replay differs from the stream launch"
+        graph_ms = timed_loop(g.replay, args.steps) / args.steps
+
     # per-kernel durations (library-side CUDA events on the same stream), separate loop
     fbp.fbp_set_profiling(plan.handle, True)
     kms = []
@@ -377,7 +397,7 @@ def measure(args, dtype, world, rank, local, dist):
     plan.close()
     del flush
     torch.cuda.empty_cache()
-    return dict(info=info, ms_step=ms_step, f_ms=f_ms, b_ms=b_ms, e2e_s=e2e_s, updates=float(B) * N * N * K,
+    return dict(info=info, graph_ms=graph_ms, ms_step=ms_step, f_ms=f_ms, b_ms=b_ms, e2e_s=e2e_s, updates=float(B) * N * N * K,
                 clocks=clk.summary(), esize=h_sino.element_size(),
                 h2d=h_sino.numel() * h_sino.element_size(), d2h=h_img.numel() * h_img.element_size(),
                 extras=extras, input_sha=input_sha)
@@ -433,7 +453,8 @@ def record(args, r, world, peaks, peaks_src, dtype):
             "e2e": {"value": total_updates / r["e2e_s"] / 1e9, "unit": UNIT, "h2d_bytes_per_step": r["h2d"],
                     "d2h_bytes_per_step": r["d2h"], "ms_per_step": r["e2e_s"] * 1e3,
                     "api": "fbp_reconstruct_host (pinned host buffers, wall clock)"},
-            "clocks": r["clocks"], "plan": info, "input_sha256": r["input_sha"]}
+            "clocks": r["clocks"], "plan": info, "input_sha256": r["input_sha"],
+            "graph_ms_per_step": r["graph_ms"]}
 
 
 def spawn_ranks(args):
@@ -492,6 +513,8 @@ def main():
             "gpu_launches": args.steps * launches_per_step,
             "clocks": rec["clocks"],
         }
+        if rec["graph_ms_per_step"] is not None:
+            line["graph_ms_per_step"] = rec["graph_ms_per_step"]
         if r64 is not None:
             rec64 = record(args, r64, world, peaks, peaks_src, "f64")
             line["f64"] = {k: rec64[k] for k in ("value", "ms_per_step", "slices_per_s", "kernels", "roofline", "e2e", "clocks")}

@@ -149,7 +149,8 @@ fbp_status fbp_reconstruct_host(fbp_plan *plan, const void *h_sino, void *h_imag
  * (any shape, e.g. one image or a whole stack).  max_val = MAX > 0.  c1, c2 < 0 select the customary
  * (0.01 MAX)^2 and (0.03 MAX)^2 (the paper does not state its constants).  d_out8: DEVICE array of
  * 8 doubles, written on the stream: MSE, PSNR (+inf when MSE = 0), SSIM, mu_x, mu_y,
- * s_x^2, s_y^2, s_xy.  fp64 sums in a fixed order: repeated calls give the same bits.  Enqueue-only;
+ * s_x^2, s_y^2, s_xy.  One pass over the two arrays (shifted fp64 moments), sums in a fixed order: repeated calls give
+ * the same bits.  Enqueue-only;
  * uses plan-owned scratch, so not concurrently with other calls on the same plan.
  */
 fbp_status fbp_metrics(fbp_plan *plan, const void *d_x, const void *d_y, long long n, double max_val,

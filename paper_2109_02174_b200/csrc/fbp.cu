@@ -86,7 +86,7 @@ struct fbp_plan {
     size_t fdk_elems = 0;
     void* d_wrow = nullptr;     // [K] dtype: angle weight / (pi/K) (fbp_set_angle_weights); NULL = uniform
 
-    double* d_mscratch = nullptr;   // fbp_metrics: [kMetricGridMax][3] CTA partials, then mid[3], ticket
+    double* d_mscratch = nullptr;   // fbp_metrics: [kMetricGridMax][6] CTA partials, then the ticket
     bool use_pdl = true;
     bool host_zero_copy = true;   // fbp_reconstruct_host: store results straight into pinned host memory
     // batch pipeline (run_pipelined): filter of slice group g+1 overlaps back-projection of group g
@@ -840,8 +840,8 @@ fbp_status create_impl(fbp_plan** out, int n_angles, int n_det, const double* an
         FBP_TRY(cudaMalloc(&p->d_tickets, sizeof(int) * nt));
         FBP_TRY(cudaMemset(p->d_tickets, 0, sizeof(int) * nt));
     }
-    FBP_TRY(cudaMalloc(&p->d_mscratch, sizeof(double) * (3 * kMetricGridMax + 8)));
-    FBP_TRY(cudaMemset(p->d_mscratch, 0, sizeof(double) * (3 * kMetricGridMax + 8)));
+    FBP_TRY(cudaMalloc(&p->d_mscratch, sizeof(double) * (fbp::kMetricSums * kMetricGridMax + 8)));
+    FBP_TRY(cudaMemset(p->d_mscratch, 0, sizeof(double) * (fbp::kMetricSums * kMetricGridMax + 8)));
     for (int i = 0; i < 4; ++i) FBP_TRY(cudaEventCreate(&p->ev[i]));
     if (tune.pipeline != 0 && max_batch >= tune.pipe_min_batch) {
         int prio_lo = 0, prio_hi = 0;
@@ -1013,16 +1013,13 @@ static cudaError_t launch_metrics(fbp_plan* p, const void* x, const void* y, lon
                                   double c1, double c2, double* d_out, cudaStream_t st)
 {
     double* partial = p->d_mscratch;
-    double* mid = p->d_mscratch + 3 * kMetricGridMax;
+    unsigned* ticket = reinterpret_cast<unsigned*>(p->d_mscratch + fbp::kMetricSums * kMetricGridMax);   // zero-initialised at fbp_create
     const int grid_max = std::min(8 * p->num_sm, kMetricGridMax);
     // at least 32 elements per thread: small inputs get few CTAs (fewer partials, fewer tickets on one counter)
     long long want = (n + 32LL * fbp::kMetricThreads - 1) / (32LL * fbp::kMetricThreads);
     const int grid = (int)(want < grid_max ? (want < 1 ? 1 : want) : grid_max);
-    const T* a = static_cast<const T*>(x);
-    const T* b = static_cast<const T*>(y);
-    unsigned* ticket = reinterpret_cast<unsigned*>(mid + 3);      // zero-initialised at fbp_create, self re-arming
-    fbp::metrics_partial_kernel<T, 0><<<grid, fbp::kMetricThreads, 0, st>>>(a, b, n, mid, partial, ticket, max_val, c1, c2, d_out);
-    fbp::metrics_partial_kernel<T, 1><<<grid, fbp::kMetricThreads, 0, st>>>(a, b, n, mid, partial, ticket, max_val, c1, c2, d_out);
+    fbp::metrics_kernel<T><<<grid, fbp::kMetricThreads, 0, st>>>(static_cast<const T*>(x), static_cast<const T*>(y), n, partial,
+                                                                 ticket, max_val, c1, c2, d_out);
     return cudaGetLastError();
 }
 
