@@ -264,7 +264,8 @@ int fbp_plan_info(const fbp_plan *plan, int *out, int n);
  *   filter CTA c          -> d_marks[8 c + s],  s = 0 start, 1 tables and first row staged, 2 partial sums done,
  *                            3 row reduced, 4 last unit stored (1-3: the CTA's first unit only)
  *   back-projector CTA c  -> d_marks[8 (F + c) + s],  F = plan_info[16],  s = 0 CTA resident, 1 past the grid
- *                            dependency, 2 first chunk landed, 3 main loop done, 4 pixels stored
+ *                            dependency, 2 first chunk landed, 3 main loop done, 4 pixels stored,
+ *                            7 the SM the CTA ran on (%smid, not a time)
  * A kernel whose records would not fit in `capacity` is not traced.  The filters carry the marks as predicated
  * stores; the back-projector runs a second instantiation of the same source with the marks compiled in (under its
  * register cap even predicated-off marks cost the main loop).  Not used by the batch pipeline's side streams.

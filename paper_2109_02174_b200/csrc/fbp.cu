@@ -51,7 +51,7 @@ struct fbp_plan {
 
     // device tables / scratch
     double2* d_cs2 = nullptr;   // [K] (cos, sin) * pix/d, fp64
-    void* d_ent = nullptr;      // [max_batch][K][planes][ent_pitch] 16-byte entries: back-projector operands
+    void* d_ent = nullptr;      // [max_batch][K][ent_pitch] 16-byte entries: back-projector operands (fbp_entries.cuh)
     void* d_part = nullptr;     // [S][max_batch][N][N] partial images when S > 1
     int* d_tickets = nullptr;   // [max_batch][tiles] arrival counters when S > 1 (self re-arming)
     void* d_hsino = nullptr;    // host-path staging (lazy)
@@ -382,7 +382,7 @@ void configure_bp(fbp_plan* p, const std::vector<double>& cs)
     p->bp_splits = S;
     const int per = (K + S - 1) / S;
 
-    const size_t entry = 4 * p->esize, rec = 4 * p->esize;
+    const size_t entry = 16, rec = 4 * p->esize;
     const size_t per_angle = (size_t)p->bp_seg * entry + rec;
     // A small launch (c CTAs per SM on average, c <= 5) is placed evenly only if no SM can hold more
     // than c of its CTAs: with programmatic dependent launch the CTAs arrive while the filter is
@@ -610,7 +610,7 @@ cudaError_t launch_bp_t(fbp_plan* p, void* image, int batch, cudaStream_t st, in
     cfg.numAttrs = 1;
     // slice0: first slice of this launch within the plan's entry buffer (`image` already points at it)
     const uint4* ent = static_cast<const uint4*>(p->d_ent) +
-                       (size_t)slice0 * p->K * fbp::EntryPlanes<T>::value * p->bp.ent_pitch;
+                       (size_t)slice0 * p->K * p->bp.ent_pitch;
     fbp::BpParams prm = p->bp;
     // trace records of the back-projector follow the filter's (fbp_set_trace)
     prm.trace = nullptr;
@@ -707,7 +707,7 @@ fbp_status run_pipelined(fbp_plan* p, const void* sino, void* image, int batch, 
     const int group = pipe_group_size(p, batch);
     const int n_groups = (batch + group - 1) / group;
     const size_t sino_slice = p->esize * (size_t)p->K * p->D, img_slice = p->esize * (size_t)p->N * p->N;
-    const size_t ent_slice = 4 * p->esize * (size_t)p->K * p->bp.ent_pitch;
+    const size_t ent_slice = 16 * (size_t)p->K * p->bp.ent_pitch;
     FBP_CUDA(p, cudaEventRecord(p->ev_fork, s));
     FBP_CUDA(p, cudaStreamWaitEvent(p->st_f, p->ev_fork, 0));
     FBP_CUDA(p, cudaStreamWaitEvent(p->st_b[0], p->ev_fork, 0));
@@ -831,7 +831,7 @@ fbp_status create_impl(fbp_plan** out, int n_angles, int n_det, const double* an
     else
         FBP_TRY(dtype == FBP_F32 ? upload_fft_tables<float>(p, 0, true) : upload_fft_tables<double>(p, 0, true));
     // entries: zero-filled once, so that the guard entries (never written by the filter) read as zeros
-    const size_t ent_bytes = 4 * p->esize * (size_t)max_batch * n_angles * p->bp.ent_pitch;
+    const size_t ent_bytes = 16 * (size_t)max_batch * n_angles * p->bp.ent_pitch;
     FBP_TRY(cudaMalloc(&p->d_ent, ent_bytes));
     FBP_TRY(cudaMemset(p->d_ent, 0, ent_bytes));
     if (p->bp_splits > 1) {

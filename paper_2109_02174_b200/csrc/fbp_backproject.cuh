@@ -5,17 +5,24 @@
 // Point symmetry.  The image grid and the detector are both centred, so the pixel (-x,-y)
 // has u' = (D-1) - u at every angle: if u = j + 1/2 + w (w in [-1/2,1/2]) then the mirror
 // pixel reads interval D-2-j with offset -w.  One thread therefore owns R pixels of the top
-// half of the image AND their R mirror pixels, computes (j, w) once, and fetches both
-// interpolation operands with ONE 16-byte (fp32) shared-memory load of the entry
+// half of the image AND their R mirror pixels, computes (j, w) once, and in fp32 fetches both
+// interpolation operands with ONE 16-byte shared-memory load of the entry
 //   E[i][j] = ( mid[j], mid[D-2-j], slope[j], -slope[D-2-j] ),
 //   mid[j] = (Q~[j]+Q~[j+1])/2,  slope[j] = Q~[j+1]-Q~[j],  Q~ = 0 outside [0, D-1]
 // so that  value = mid_a + w slope_a  and  mirror value = mid_b + w nslope_b; in fp32 that is
 // one packed FFMA2 + one packed FADD2 on the (pixel, mirror) accumulator pair.
-// In fp64 the entry is split into two 16-byte planes (mids, slopes) so that consecutive
-// entries stay 16 bytes apart (a 32-byte entry would 2-way bank-conflict every LDS.128).
+// In fp64 the 16-byte unit of interval j holds the NEAR end points (Q~[j], Q~[D-1-j]) of the interval and
+// of its mirror; the far end points are the next unit:  value = near (1-w) + far w,  w = u - floor(u) in [0,1).
+// A thread's R pixels step by s = sin(theta) pix/d along its column; where 0 <= s <= 1 - 2^-40 (every angle of
+// [0, pi] at pix <= d) consecutive pixels fall into the same or the next interval, so the thread WALKS: it keeps
+// `near` in registers (the previous pixel's near or far, one select) and loads only `far` -- one LDS.128 per
+// pixel pair instead of two, 8 instead of 16 bytes of shared-memory operands per update.  Angles outside that
+// range (the producer flags every staged chunk) load both end points.  (In fp32 the same walk is slower than
+// the (mid, slope) entry: the selects and the extra subtract cost more issue slots than the saved wavefronts --
+// measured.)
 // The entries are produced by the filter epilogue (fbp_reconstruct) or entries_kernel
-// (fbp_backproject) into a plan-owned buffer [batch][K][planes][pitch] with >= L+1 zero
-// guard entries on both sides (fbp_filter.cuh, "entries").
+// (fbp_backproject) into a plan-owned buffer [batch][K][pitch] with >= L+1 zero
+// guard entries on both sides (fbp_entries.cuh).
 //
 // A CTA owns a tile of 32 x (WY*R) primary pixels and a contiguous range of angles (split s
 // of S).  Its warps form WA groups of WY warps; group g takes every WA-th angle, so one small
@@ -25,9 +32,10 @@
 // fp64, the tile-local base b = u(tile origin) - j0 - 1/2 (fp32 coordinates stay below 64:
 // ulp <= 3.8e-6) and issues one TMA bulk copy (cp.async.bulk, completion on an mbarrier) of
 // the L entries starting at j0 into the other stage.
-// Per update pair:  u' = b + lx cos + ly sin;  t = u' + M (M = 1.5*2^23 | 1.5*2^52, round to
-// nearest);  e = bits(t) - bits(M);  w = u' - (t - M);  one LDS.128;  2 FMA + 2 ADD.
-// A tie in the rounding picks either neighbouring interval with the same interpolated value.
+// Per update pair, fp32:  u' = b + lx cos + ly sin;  t = u' + M (M = 1.5*2^23, round to nearest);
+// e = bits(t) - bits(M);  w = u' - (t - M);  one LDS.128;  2 FMA + 2 ADD.  A tie in the rounding picks
+// either neighbouring interval with the same interpolated value.  fp64: b carries no -1/2 and the add
+// rounds DOWN (M = 1.5*2^52), so e = floor(u'), w = u' - e in [0, 1).
 // One owner per pixel, ascending angles => bit-identical runs.  With S > 1 (one small slice
 // would otherwise leave most of the 148 SMs idle) the S CTAs of a tile each write their
 // partial tile to a scratch image [S][batch][N][N] and take a ticket (one atomicAdd per CTA on
@@ -75,13 +83,12 @@ template <typename T> struct alignas(4 * sizeof(T)) AngleRec { T c, s, b, pad; }
 // ---- the per-update arithmetic: (pixel, mirror pixel) accumulator pair ---------------------
 // fp32: packed pair in one 64-bit register; LDS.128 -> (mids, slopes) as two packed pairs;
 //       t = slopes * (w, w) + mids  (FFMA2, scalar w broadcast);  acc += t  (FADD2).
-// fp64: two 16-byte planes -> two LDS.128; scalar DFMA + DADD per pixel.
+// fp64: near/far end points (two LDS.128, or one when walking); 1 DADD + 4 DFMA per pixel pair.
 template <typename T> struct PairAcc;
 template <> struct PairAcc<float> {
     unsigned long long v;
-    static constexpr int kPlanes = 1;
     __device__ __forceinline__ void zero() { v = 0ull; }
-    __device__ __forceinline__ void update(unsigned addr, unsigned /*plane_stride*/, float w)
+    __device__ __forceinline__ void update(unsigned addr, float w)
     {
 #ifndef FBP_SCALAR_PAIR
         unsigned long long m2, s2, w2, t;
@@ -101,21 +108,23 @@ template <> struct PairAcc<float> {
 };
 template <> struct PairAcc<double> {
     double va, vb;
-    static constexpr int kPlanes = 2;
     __device__ __forceinline__ void zero() { va = 0.0; vb = 0.0; }
-    __device__ __forceinline__ void update(unsigned addr, unsigned plane_stride, double w)
+    // near (1-w) + far w for the pixel and its mirror
+    __device__ __forceinline__ void lerp(double na, double nb, double fa, double fb, double w)
     {
-        double ma, mb, sa, sb;
-        asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(ma), "=d"(mb) : "r"(addr));
-        asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(sa), "=d"(sb) : "r"(addr + plane_stride));
-        va += fma(w, sa, ma);
-        vb += fma(w, sb, mb);
+        const double omw = 1.0 - w;
+        va = fma(na, omw, va); vb = fma(nb, omw, vb);
+        va = fma(fa, w, va);   vb = fma(fb, w, vb);
     }
     __device__ __forceinline__ double a() const { return va; }
     __device__ __forceinline__ double b() const { return vb; }
 };
+__device__ __forceinline__ void lds_f64x2(double& x, double& y, unsigned addr)
+{
+    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(x), "=d"(y) : "r"(addr));
+}
 
-// cs2: [K] pairs (cos*pix/d, sin*pix/d) in fp64.  E: 16-byte entry units [batch][K][planes][pitch].
+// cs2: [K] pairs (cos*pix/d, sin*pix/d) in fp64.  E: 16-byte entry units [batch][K][pitch].
 // Grid (tiles, S, batch).  image: [batch][N][N], fully written, scaled by pi/K.
 // part: scratch [S][batch][N][N] and tickets: [batch][tiles] zero-initialised counters (S > 1 only).
 // TRACE: the instantiation launched while fbp_set_trace is on (the marks are compiled out of the other one: under its
@@ -140,14 +149,15 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
                    T* __restrict__ part, int* __restrict__ tickets, BpParams prm)
 {
     constexpr int TH = WY * R;
-    constexpr int NP = PairAcc<T>::kPlanes;
     constexpr int NW = WY * WA;          // consumer warps; warp NW is the producer
     constexpr int NS = kBpStages;
     extern __shared__ __align__(128) unsigned char bp_smem_raw[];
-    // layout: full[NS], empty[NS] mbarriers (64 B) | rec[NS][chunk] | pad to 128 |
-    //         seg[NS stages][planes][chunk][L] x 16 B
+    // layout: full[NS], empty[NS] mbarriers, walk[NS] flags (64 B) | rec[NS][chunk] | pad to 128 |
+    //         seg[NS stages][chunk][L] x 16 B
     const unsigned bar_full = smem_u32(bp_smem_raw);
     const unsigned bar_empty = bar_full + 8u * NS;
+    static_assert(16 * NS + 4 * NS <= 64, "barriers and flags share the 64-byte header");
+    volatile int* walk_flag = reinterpret_cast<volatile int*>(bp_smem_raw + 16 * NS);   // fp64: every angle of the stage may be walked
     AngleRec<T>* rec = reinterpret_cast<AngleRec<T>*>(bp_smem_raw + 64);
     unsigned char* seg_ptr = bp_smem_raw + 64 + NS * (size_t)prm.chunk * sizeof(AngleRec<T>);
     seg_ptr += (128 - (reinterpret_cast<uintptr_t>(seg_ptr) & 127)) & 127;
@@ -155,15 +165,21 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned cta_id = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
-    if (TRACE) trace_mark(prm.trace, cta_id, 0);               // CTA resident
+    if (TRACE) {
+        trace_mark(prm.trace, cta_id, 0);                       // CTA resident
+        if (prm.trace != nullptr && threadIdx.x == 0) {         // slot 7: the SM this CTA runs on (placement and fairness studies)
+            unsigned smid;
+            asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+            prm.trace[(size_t)cta_id * 8 + 7] = smid;
+        }
+    }
     const bool producer = warp == NW;
     const int wy = warp % WY, wa = producer ? WA : warp / WY;
     const int tile = blockIdx.x;
     const int ty = tile / prm.tiles_x, tx = tile - ty * prm.tiles_x;
     const int split = blockIdx.y, b = blockIdx.z;
     const int K = prm.n_angles, N = prm.image_n, L = prm.seg_len, S = prm.n_splits;
-    const unsigned plane_stride = (unsigned)(prm.chunk * L * 16);
-    const unsigned stage_stride = plane_stride * NP;
+    const unsigned stage_stride = (unsigned)(prm.chunk * L * 16);
 
     const int per = (K + S - 1) / S;
     const int a_begin = split * per;
@@ -192,24 +208,29 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
         // ---- producer warp: per angle, the tile-local record (fp64) and one TMA bulk copy ----
         const double x0 = (double)(tx * 32) - prm.c_n;
         const double y0 = (double)(ty * TH) - prm.c_n;
-        const uint4* Eb = E + (size_t)b * K * NP * prm.ent_pitch;
+        const uint4* Eb = E + (size_t)b * K * prm.ent_pitch;
         for (int k = 0; k < n_chunks; ++k) {
             const int st = k % NS;
-            if (k >= NS) mbar_wait(bar_empty + 8u * st, (unsigned)((k / NS - 1) & 1));  // stage released
             const int a0 = a_begin + k * prm.chunk;
             const int na = min(prm.chunk, a_end - a0);
             const unsigned bar = bar_full + 8u * st;
-            for (int a = lane; a < na; a += 32) {
-                AngleRec<T> rc;
+            // lane a's record and source address are computed BEFORE waiting for the stage to be released:
+            // the table read and the fp64 arithmetic overlap the consumers' work on the chunks in flight
+            // (chunk <= 32: one angle per lane)
+            AngleRec<T> rc;
+            const uint4* src = Eb;
+            bool walk_ok = true;
+            if (lane < na) {
                 long long off;            // first staged entry of this angle's row, in entries from the row start
-                const double2 cs = cs2[a0 + a];
+                const double2 cs = cs2[a0 + lane];
                 const double ub = x0 * cs.x + y0 * cs.y + prm.c_d;
                 const double umin = ub + fmin(0.0, 31.0 * cs.x) + fmin(0.0, (double)(TH - 1) * cs.y);
                 const double fl = floor(umin) - 1.0;
                 // the window [j0, j0+L) must lie inside the guarded row [-guard, pitch-guard)
                 if (fl >= -(double)prm.ent_guard && fl <= (double)(prm.ent_pitch - prm.ent_guard - L)) {
                     off = (long long)fl + prm.ent_guard;
-                    rc.c = (T)cs.x; rc.s = (T)cs.y; rc.b = (T)(ub - fl - 0.5);
+                    rc.c = (T)cs.x; rc.s = (T)cs.y;
+                    rc.b = sizeof(T) == 4 ? (T)(ub - fl - 0.5) : (T)(ub - fl);
                 } else {
                     // the tile projects entirely off the detector at this angle: stage the
                     // all-zero left guard and pin every pixel to entry 1 of it
@@ -217,17 +238,22 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
                     rc.c = T(0); rc.s = T(0); rc.b = T(1);
                 }
                 rc.pad = T(0);
-                rec[st * prm.chunk + a] = rc;
-                const uint4* src = Eb + (size_t)(a0 + a) * NP * prm.ent_pitch + off;
-#pragma unroll
-                for (int pl = 0; pl < NP; ++pl)
-                    tma_load_1d(seg + st * stage_stride + pl * plane_stride + (unsigned)(a * L * 16),
-                                src + (size_t)pl * prm.ent_pitch, (unsigned)(L * 16), bar);
+                src = Eb + (size_t)(a0 + lane) * prm.ent_pitch + off;
+                // fp64: may the consumers walk along their column at this angle?  (0 <= step < 1 with a margin far
+                // above the rounding of fma(r, s, u0): the interval index then never moves by more than 1)
+                walk_ok = cs.y >= 0.0 && cs.y <= 1.0 - 0x1p-40;
             }
+            if (sizeof(T) == 8) walk_ok = __all_sync(0xffffffffu, walk_ok);
+            if (k >= NS) mbar_wait(bar_empty + 8u * st, (unsigned)((k / NS - 1) & 1));  // stage released
+            if (lane < na) {
+                rec[st * prm.chunk + lane] = rc;
+                tma_load_1d(seg + st * stage_stride + (unsigned)(lane * L * 16), src, (unsigned)(L * 16), bar);
+            }
+            if (sizeof(T) == 8 && lane == 0) walk_flag[st] = walk_ok ? 1 : 0;
             // every lane's records are written before lane 0's (releasing) arrival, so a warp
             // that sees the phase complete also sees the records
             __syncwarp();
-            if (lane == 0) mbar_arrive_expect_tx(bar, (unsigned)(na * L * 16 * NP));
+            if (lane == 0) mbar_arrive_expect_tx(bar, (unsigned)(na * L * 16));
         }
     } else {
         // ---- consumer warps: no block-wide barrier, only data (full) waits ----
@@ -240,17 +266,66 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
             if (TRACE && k == 0) trace_mark(prm.trace, cta_id, 2);   // first chunk landed (thread 0 is a consumer)
             const AngleRec<T>* rk = rec + st * prm.chunk;
             const unsigned segk = seg + st * stage_stride - Magic<T>::kBits * 16u;  // bits(M) folded in
+            if constexpr (sizeof(T) == 4) {
 #pragma unroll 2
-            for (int a = wa; a < na; a += WA) {
-                const AngleRec<T> rc = rk[a];
-                const unsigned rowbase = segk + (unsigned)(a * L * 16);
-                const T u0 = fma(lx, rc.c, fma(ly, rc.s, rc.b));
+                for (int a = wa; a < na; a += WA) {
+                    const AngleRec<T> rc = rk[a];
+                    const unsigned rowbase = segk + (unsigned)(a * L * 16);
+                    const T u0 = fma(lx, rc.c, fma(ly, rc.s, rc.b));
 #pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    const T u = fma((T)r, rc.s, u0);
-                    const T t = u + M;
-                    const T w = u - (t - M);
-                    acc[r].update(rowbase + Magic<T>::bits(t) * 16u, plane_stride, w);
+                    for (int r = 0; r < R; ++r) {
+                        const T u = fma((T)r, rc.s, u0);
+                        const T t = u + M;
+                        const T w = u - (t - M);
+                        acc[r].update(rowbase + Magic<T>::bits(t) * 16u, w);
+                    }
+                }
+            } else if (walk_flag[st] != 0) {
+                // walk: `near` of pixel r is the previous pixel's near (same interval) or far (next interval)
+#pragma unroll 2
+                for (int a = wa; a < na; a += WA) {
+                    const AngleRec<T> rc = rk[a];
+                    const unsigned rowbase = segk + (unsigned)(a * L * 16);
+                    const double u0 = fma(lx, rc.c, fma(ly, rc.s, rc.b));
+                    double na_ = 0.0, nb_ = 0.0, pa = 0.0, pb = 0.0;
+                    unsigned pe = 0u;
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        const double u = fma((double)r, rc.s, u0);
+                        const double t = __dadd_rd(u, M);
+                        const double w = u - (t - M);
+                        const unsigned e = Magic<T>::bits(t);
+                        const unsigned addr = rowbase + e * 16u;
+                        double fa, fb;
+                        lds_f64x2(fa, fb, addr + 16u);
+                        if (r == 0) {
+                            lds_f64x2(na_, nb_, addr);
+                        } else {
+                            const bool moved = e != pe;
+                            na_ = moved ? pa : na_;
+                            nb_ = moved ? pb : nb_;
+                        }
+                        acc[r].lerp(na_, nb_, fa, fb, w);
+                        pe = e; pa = fa; pb = fb;
+                    }
+                }
+            } else {
+#pragma unroll 2
+                for (int a = wa; a < na; a += WA) {
+                    const AngleRec<T> rc = rk[a];
+                    const unsigned rowbase = segk + (unsigned)(a * L * 16);
+                    const double u0 = fma(lx, rc.c, fma(ly, rc.s, rc.b));
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        const double u = fma((double)r, rc.s, u0);
+                        const double t = __dadd_rd(u, M);
+                        const double w = u - (t - M);
+                        const unsigned addr = rowbase + Magic<T>::bits(t) * 16u;
+                        double na_, nb_, fa, fb;
+                        lds_f64x2(na_, nb_, addr);
+                        lds_f64x2(fa, fb, addr + 16u);
+                        acc[r].lerp(na_, nb_, fa, fb, w);
+                    }
                 }
             }
             __syncwarp();

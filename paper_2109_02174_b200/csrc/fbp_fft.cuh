@@ -291,14 +291,14 @@ fft_filter_kernel(const T* __restrict__ Pin, T* __restrict__ Q, uint4* __restric
                 for (int n = tid; n < D; n += nthr) q[n] = yz[n + 1 + guard];
             }
             if (E) {
-                uint4* erow = E + row * EntryPlanes<T>::value * pitch;
+                uint4* erow = E + row * pitch;
                 const bool scaled = wrow != nullptr;
                 const T m = scaled ? wrow[ra + h] : T(1);
                 for (int i = guard - 1 + tid; i <= guard + D - 1; i += nthr) {
                     T a0 = yz[i + 1], a1 = yz[i + 2];
                     T b0 = yz[pitch - 1 - i], b1 = yz[pitch - i];
                     if (scaled) { a0 *= m; a1 *= m; b0 *= m; b1 *= m; }
-                    store_entry(erow, pitch, i, T(0.5) * (a0 + a1), T(0.5) * (b0 + b1), a1 - a0, b0 - b1);
+                    store_entry(erow, i, a0, a1, b0, b1);
                 }
             }
         }

@@ -298,17 +298,15 @@ filter3_kernel(const T* __restrict__ P, T* __restrict__ Q, uint4* __restrict__ E
             // j in [j_beg, j_end) and writes both entries of each pair
             const int j_beg = u == 0 ? -1 : nL0;
             const int j_end = inner ? D / 2 : nL0 + 15 * W2;        // floor(D/2) = number of left members >= 0
-            uint4* erow = E + (size_t)row * EntryPlanes<T>::value * prm.ent_pitch;
+            uint4* erow = E + (size_t)row * prm.ent_pitch;
             const bool scaled = wrow != nullptr;
             const T m = scaled ? wrow[row % n_angles] : T(1);
             for (int j = j_beg + tid; j < j_end; j += nthr) {
                 const int jm = D - 2 - j;
                 T a0v = q_at(j), a1v = q_at(j + 1), b0v = q_at(jm), b1v = q_at(jm + 1);
                 if (scaled) { a0v *= m; a1v *= m; b0v *= m; b1v *= m; }
-                const T mid_a = T(0.5) * (a0v + a1v), mid_b = T(0.5) * (b0v + b1v);
-                const T sl_a = a1v - a0v, sl_b = b1v - b0v;
-                store_entry(erow, prm.ent_pitch, j + prm.ent_guard, mid_a, mid_b, sl_a, -sl_b);
-                if (jm != j) store_entry(erow, prm.ent_pitch, jm + prm.ent_guard, mid_b, mid_a, sl_b, -sl_a);
+                store_entry(erow, j + prm.ent_guard, a0v, a1v, b0v, b1v);
+                if (jm != j) store_entry(erow, jm + prm.ent_guard, b0v, b1v, a0v, a1v);
             }
         }
     }
