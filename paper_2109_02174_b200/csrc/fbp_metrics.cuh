@@ -23,6 +23,7 @@ namespace fbp {
 
 constexpr int kMetricThreads = 256;
 constexpr int kMetricSums = 6;
+constexpr int kMetricU = 4;      // 16-byte vectors per array, thread and pipeline stage
 
 // partial: [gridDim.x][6] doubles.  ticket: zero-initialised, self re-arming.  out: 8 doubles.
 template <typename T>
@@ -37,7 +38,7 @@ metrics_kernel(const T* __restrict__ x, const T* __restrict__ y, long long n, do
         s[0] += u; s[1] += v;
         s[2] = fma(u, u, s[2]); s[3] = fma(v, v, s[3]); s[4] = fma(u, v, s[4]); s[5] = fma(e, e, s[5]);
     };
-    // 16-byte loads, four in flight per array and thread; the element -> thread map is fixed by (n, grid)
+    // 16-byte loads; the element -> thread map is fixed by (n, grid)
     constexpr int V = 16 / (int)sizeof(T);
     const bool vec = ((reinterpret_cast<uintptr_t>(x) | reinterpret_cast<uintptr_t>(y)) & 15u) == 0;
     const long long nvec = vec ? n / V : 0;
@@ -45,25 +46,36 @@ metrics_kernel(const T* __restrict__ x, const T* __restrict__ y, long long n, do
     const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const uint4* xv = reinterpret_cast<const uint4*>(x);
     const uint4* yv = reinterpret_cast<const uint4*>(y);
+    // software pipeline: the loads of the next group of kMetricU vectors per array are in flight while the current
+    // group is accumulated (a warp that computes after waiting for its loads leaves HBM idle a third of the time);
+    // the accumulation order of a thread -- ascending index -- does not depend on the grouping
+    constexpr int U = kMetricU;
+    uint4 a[U], b[U];
     long long i = t0;
-    for (; i + 3 * stride < nvec; i += 4 * stride) {
-        uint4 a[4], b[4];
+    auto load = [&](long long at) {
 #pragma unroll
-        for (int u = 0; u < 4; ++u) { a[u] = __ldg(xv + i + u * stride); b[u] = __ldg(yv + i + u * stride); }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const T* pa = reinterpret_cast<const T*>(&a[u]);
-            const T* pb = reinterpret_cast<const T*>(&b[u]);
-#pragma unroll
-            for (int e = 0; e < V; ++e) add((double)pa[e], (double)pb[e]);
+        for (int u = 0; u < U; ++u) {
+            const long long k = at + u * stride;
+            if (k < nvec) { a[u] = __ldg(xv + k); b[u] = __ldg(yv + k); }
         }
-    }
-    for (; i < nvec; i += stride) {
-        const uint4 a = __ldg(xv + i), b = __ldg(yv + i);
-        const T* pa = reinterpret_cast<const T*>(&a);
-        const T* pb = reinterpret_cast<const T*>(&b);
+    };
+    if (i < nvec) load(i);
+    while (i < nvec) {
+        uint4 ca[U], cb[U];
 #pragma unroll
-        for (int e = 0; e < V; ++e) add((double)pa[e], (double)pb[e]);
+        for (int u = 0; u < U; ++u) { ca[u] = a[u]; cb[u] = b[u]; }
+        const long long nxt = i + U * stride;
+        if (nxt < nvec) load(nxt);
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            if (i + u * stride < nvec) {
+                const T* pa = reinterpret_cast<const T*>(&ca[u]);
+                const T* pb = reinterpret_cast<const T*>(&cb[u]);
+#pragma unroll
+                for (int e = 0; e < V; ++e) add((double)pa[e], (double)pb[e]);
+            }
+        }
+        i = nxt;
     }
     for (long long k = nvec * V + t0; k < n; k += stride) add((double)x[k], (double)y[k]);   // tail / unaligned
 #pragma unroll
