@@ -79,6 +79,10 @@ template <> struct Magic<double> {
     static constexpr unsigned kBits = 0u;
 };
 
+// a + b rounded toward -infinity: with b = Magic::m() the floor of a (|a| < 2^22 | 2^51) lands in the low mantissa bits
+__device__ __forceinline__ float add_rd(float a, float b) { return __fadd_rd(a, b); }
+__device__ __forceinline__ double add_rd(double a, double b) { return __dadd_rd(a, b); }
+
 template <typename T> struct alignas(4 * sizeof(T)) AngleRec { T c, s, b, pad; };
 // ---- the per-update arithmetic: (pixel, mirror pixel) accumulator pair ---------------------
 // fp32: packed pair in one 64-bit register; LDS.128 -> (mids, slopes) as two packed pairs;

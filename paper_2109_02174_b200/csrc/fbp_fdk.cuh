@@ -38,52 +38,93 @@ fdk_weight_kernel(const T* __restrict__ p, T* __restrict__ out, long long n, int
     out[e] = (T)((double)p[e] * (sad * rsqrt(sad * sad + a * a + b * b)));
 }
 
-constexpr int kFdkZT = 8;        // voxels per thread along z
 
-// Q: [K][n_b][n_a] filtered, weighted projections.  cs2: [K] (cos, sin) * pix/d_a (fp64).  vol: [n_z][N][N].
-// Grid (ceil(N/32), ceil(N/4), ceil(n_z/ZT)), block (32, 4): thread = one (x, y) and ZT consecutive z.
+// The back-projector's operands: 2 x 2 neighbourhoods ("quads") of the filtered projections with zero borders,
+//   P4[m][i'][j'] = ( Q~[i][j], Q~[i][j+1], Q~[i+1][j], Q~[i+1][j+1] ),  i = i'-1, j = j'-1,
+//   i' in [0, n_b+2), j' in [0, n_a+2),  Q~ = 0 outside the detector,
+// so that a bilinear sample at (ua, ub) clamped to [-1, n_a] x [-1, n_b] is ONE aligned 16-byte load (fp32; two in
+// fp64) at one address, with no bounds test: whatever lies outside the detector reads as zero.  Four times the bytes
+// of the plain projections; per angle they are read by every CTA at about the same time and stay in L2.
+template <typename T> struct alignas(4 * sizeof(T)) FdkQuad { T q00, q01, q10, q11; };
+
+// One thread per quad.
 template <typename T>
-__global__ void __launch_bounds__(128)
-fdk_backproject_kernel(const T* __restrict__ Q, T* __restrict__ vol, const double2* __restrict__ cs2, FdkParams prm)
+__global__ void __launch_bounds__(256)
+fdk_quads_kernel(const T* __restrict__ Q, FdkQuad<T>* __restrict__ P4, long long n, int n_a, int n_b)
 {
-    const int c = blockIdx.x * 32 + threadIdx.x, r = blockIdx.y * 4 + threadIdx.y, k0 = blockIdx.z * kFdkZT;
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    const int pa = n_a + 2, pb = n_b + 2;
+    const int jp = (int)(e % pa), ip = (int)((e / pa) % pb);
+    const long long m = e / ((long long)pa * pb);
+    const int i = ip - 1, j = jp - 1;
+    auto at = [&](int ii, int jj) -> T {
+        return (ii >= 0 && ii < n_b && jj >= 0 && jj < n_a) ? Q[((size_t)m * n_b + ii) * n_a + jj] : T(0);
+    };
+    FdkQuad<T> v;
+    v.q00 = at(i, j); v.q01 = at(i, j + 1); v.q10 = at(i + 1, j); v.q11 = at(i + 1, j + 1);
+    P4[e] = v;
+}
+
+__device__ __forceinline__ FdkQuad<float> ldg_quad(const FdkQuad<float>* p)
+{
+    const float4 v = __ldg(reinterpret_cast<const float4*>(p));
+    return FdkQuad<float>{v.x, v.y, v.z, v.w};
+}
+__device__ __forceinline__ FdkQuad<double> ldg_quad(const FdkQuad<double>* p)
+{
+    const double2 a = __ldg(reinterpret_cast<const double2*>(p)), b = __ldg(reinterpret_cast<const double2*>(p) + 1);
+    return FdkQuad<double>{a.x, a.y, b.x, b.y};
+}
+
+// P4: the quads above.  cs2: [K] (cos, sin) * pix/d_a (fp64).  vol: [n_z][N][N].
+// Grid (ceil(N/32), ceil(N/4), ceil(n_z/ZT)), block (32, 4): thread = one (x, y) and ZT consecutive z (ZT = 16, or 8 for
+// thin volumes).  Per (x, y, angle), in fp64 and shared by the ZT voxels: column coordinate ua (clamped, floor by the round-down add of
+// 1.5 * 2^52), magnification, weight.  Per voxel, in the working precision: ub = mag z + c_b clamped to [-1, n_b], floor
+// and fraction by the same trick (no F2I / I2F: those run at a quarter of the issue rate), one quad load, three lerps.
+template <typename T, int ZT>
+__global__ void __launch_bounds__(128)
+fdk_backproject_kernel(const FdkQuad<T>* __restrict__ P4, T* __restrict__ vol, const double2* __restrict__ cs2, FdkParams prm)
+{
+    const int c = blockIdx.x * 32 + threadIdx.x, r = blockIdx.y * 4 + threadIdx.y, k0 = blockIdx.z * ZT;
     const int N = prm.image_n, n_a = prm.n_a, n_b = prm.n_b;
     if (c >= N || r >= N) return;
     const double xi = (double)c - prm.c_n, yi = (double)r - prm.c_n;
     const T M = Magic<T>::m();
-    T zk[kFdkZT], acc[kFdkZT];
+    const double M64 = Magic<double>::m();
+    T acc[ZT];
 #pragma unroll
-    for (int z = 0; z < kFdkZT; ++z) { zk[z] = (T)(((double)(k0 + z) - prm.c_z) * prm.rz); acc[z] = T(0); }
-    const size_t plane = (size_t)n_b * n_a;
+    for (int z = 0; z < ZT; ++z) acc[z] = T(0);
+    const T zk0 = (T)(((double)k0 - prm.c_z) * prm.rz), rz = (T)prm.rz;     // z of voxel k0 + z: zk0 + z rz (detector rows)
+    const int pa = n_a + 2;
+    const unsigned plane = (unsigned)(n_b + 2) * (unsigned)pa;      // quads per angle (< 2^31: checked by the caller)
+    const T ub_hi = (T)n_b, cb = (T)prm.c_b;
+    const double ua_hi = (double)n_a;
     for (int m = 0; m < prm.n_angles; ++m) {
         const double2 cs = cs2[m];
-        // per (x, y, angle), in fp64 (shared by the ZT voxels): column coordinate and magnification
         const double t = xi * cs.x + yi * cs.y, s = yi * cs.x - xi * cs.y;
         const double mag = prm.sad_a / (prm.sad_a + s);
-        const double ua = mag * t + prm.c_a;
-        const double fa = floor(ua);
-        const int ja = (int)fa;
-        const T wa = (T)(ua - fa), w2 = (T)(mag * mag), mg = (T)mag, cb = (T)prm.c_b;
-        const T* Qm = Q + (size_t)m * plane;
-        const bool in0 = ja >= 0 && ja < n_a, in1 = ja + 1 >= 0 && ja + 1 < n_a;
-        if (!in0 && !in1) continue;
+        const double ua = fmin(fmax(mag * t + prm.c_a, -1.0), ua_hi);
+        const double ta = __dadd_rd(ua, M64);
+        const int ja = __double2loint(ta);                           // floor(ua) in [-1, n_a]
+        const T wa = (T)(ua - (ta - M64)), w2 = (T)(mag * mag), mg = (T)mag;
+        // quads of column ja (buffer rows: detector row i is row i + 1, so the row index floor(ub) + 1 is in [0, n_b + 1])
+        const FdkQuad<T>* col = P4 + (size_t)m * plane + (unsigned)(ja + 1);
+        const T ub0 = fma(mg, zk0, cb), du = mg * rz;
 #pragma unroll
-        for (int z = 0; z < kFdkZT; ++z) {
-            const T ub = fma(mg, zk[z], cb);
-            const T tb = ub + M;
-            const int ib = (int)(Magic<T>::bits(tb) - Magic<T>::kBits) - (tb - M > ub ? 1 : 0);   // floor(ub)
-            const T wb = ub - (T)ib;
-            const T* row0 = Qm + (size_t)ib * n_a + ja;
-            const bool r0 = ib >= 0 && ib < n_b, r1 = ib + 1 >= 0 && ib + 1 < n_b;
-            const T q00 = (r0 && in0) ? __ldg(row0) : T(0), q01 = (r0 && in1) ? __ldg(row0 + 1) : T(0);
-            const T q10 = (r1 && in0) ? __ldg(row0 + n_a) : T(0), q11 = (r1 && in1) ? __ldg(row0 + n_a + 1) : T(0);
-            const T v0 = fma(wa, q01 - q00, q00), v1 = fma(wa, q11 - q10, q10);
+        for (int z = 0; z < ZT; ++z) {
+            const T ub = fmin(fmax(fma((T)z, du, ub0), T(-1)), ub_hi);
+            const T tb = add_rd(ub, M);
+            const unsigned ibp = Magic<T>::bits(tb) - (Magic<T>::kBits - 1u);   // floor(ub) + 1
+            const T wb = ub - (tb - M);
+            const FdkQuad<T> q = ldg_quad(col + (size_t)(ibp * (unsigned)pa));
+            const T v0 = fma(wa, q.q01 - q.q00, q.q00), v1 = fma(wa, q.q11 - q.q10, q.q10);
             acc[z] = fma(w2, fma(wb, v1 - v0, v0), acc[z]);
         }
     }
     const T sc = (T)prm.scale;
 #pragma unroll
-    for (int z = 0; z < kFdkZT; ++z)
+    for (int z = 0; z < ZT; ++z)
         if (k0 + z < prm.n_z) vol[((size_t)(k0 + z) * N + r) * N + c] = acc[z] * sc;
 }
 
