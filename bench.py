@@ -416,7 +416,10 @@ def record(args, r, world, peaks, peaks_src, dtype):
     achieved = bp_gups * 1e9 * FP_INSTR_PER_UPDATE / 1e12
     # co-limiter: every update needs two operands of the dtype from shared memory (128 B/clk/SM), whatever the packing
     smem_peak_tbs = n_sm * 128 * sm_max_mhz * 1e6 / 1e12
-    smem_tbs = bp_gups * 1e9 * 2 * r["esize"] / 1e12
+    # bytes of shared-memory operands per update: fp32 one 16-byte (mid, slope) unit per pixel pair; fp64 one 16-byte
+    # `far` unit per pixel pair (the column walk keeps `near` in registers)
+    smem_bytes_per_update = 8.0
+    smem_tbs = bp_gups * 1e9 * smem_bytes_per_update / 1e12
     filt_bytes = 2.0 * cfg.batch * cfg.n_angles * cfg.n_det * r["esize"]
     kern = {"filter_ms": r["f_ms"], "backproject_ms": r["b_ms"], "backproject_gupdates_per_s": bp_gups,
             "filter_kind": {1: "direct", 2: "fft"}.get(info.get("filter_kind"), "?"),
@@ -442,9 +445,10 @@ def record(args, r, world, peaks, peaks_src, dtype):
             "traffic": ncu_traffic(args.config, dtype, "backproject"),
             "co_limit": {"bound": "smem", "achieved": smem_tbs, "peak": smem_peak_tbs, "unit": "TB/s of shared-memory operands",
                          "frac": smem_tbs / smem_peak_tbs,
-                         "note": "2 operands per update whatever the packing: 16 (fp32) / 8 (fp64) updates per clock and SM; "
-                                 "this is the ceiling the kernel sits on (DESIGN.md 6.2), at %.3f of the issue roofline"
-                                 % (smem_peak_tbs / (2 * r["esize"]) / (peak_tinstr / FP_INSTR_PER_UPDATE))},
+                         "note": "8 bytes of shared-memory operands per update = 16 updates per clock and SM, %.3f of the "
+                                 "issue roofline: the ceiling the fp32 kernel sits on; not binding in fp64 since the "
+                                 "column walk (FP64 pipe / issue bound; DESIGN.md 6.2)"
+                                 % (smem_peak_tbs / smem_bytes_per_update / (peak_tinstr / FP_INSTR_PER_UPDATE))},
             "how": "%d FP instr/update (SURVEY 8(d)) x updates per launch / mean CUDA-event duration of the "
                    "back-projection launch(es); peak = %d SMs x %d lanes x %.0f MHz (%s sm_max_mhz)"
                    % (FP_INSTR_PER_UPDATE, n_sm, lanes, sm_max_mhz, peaks_src)}
