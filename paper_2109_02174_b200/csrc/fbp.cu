@@ -81,7 +81,7 @@ struct fbp_plan {
     } fft;
     int filter_kind = 1;        // 1 direct form, 2 FFT form
     int window = 0;             // fbp_set_window; 0 = Ram-Lak
-    void* d_xt = nullptr;       // 2 x [max_batch][N][N + 2 pad] dtype: padded image and padded transpose for fbp_project
+    void* d_xt = nullptr;       // 2 x [max_batch][N][pitch] pairs: padded image and padded transpose, each interleaved with its point mirror (fbp_project)
     void* d_fdk = nullptr;      // fbp_fdk_reconstruct: weighted | filtered cone-beam projections [K][n_rows][n_det], then the
                                 // back-projector's zero-bordered 2 x 2 quads [K][n_rows + 2][n_det + 2][4]
     size_t fdk_elems = 0;
@@ -1061,28 +1061,40 @@ fbp_status fbp_project(fbp_plan* p, const void* d_image, void* d_sino, int batch
     if (st != FBP_OK) return st;
     if (d_image == d_sino) return fail(p, FBP_EINVAL, "fbp_project: input and output may not alias");
     DeviceGuard guard(p->device);
-    // zero pad of the staged lines: the widest run is 2 E + 1 pixels, E <= ceil(sqrt(2) d/pix + 1/2) - 1
-    const int e_max = (int)std::ceil(std::sqrt(2.0) * p->d / p->pix + 0.5) - 1;
-    const int pad = round_up(2 * e_max + 2, 4);            // round(p*) is clamped to [-(E+1), N+E], the run adds +-E
-    const size_t plane = (size_t)p->N * (p->N + 2 * pad);
-    if (!p->d_xt) FBP_CUDA(p, cudaMalloc(&p->d_xt, p->esize * 2 * (size_t)p->max_batch * plane));
+    // geometry of the staged copies and of the projector's windows (fbp_project.cuh): the widest run is 2 E + 1 pixels,
+    // E <= ceil(sqrt(2) d/pix + 1/2) - 1; a CTA's 128 bins span at most 127 sqrt(2) d/pix pixels of a line
+    const double inv_max = std::sqrt(2.0) * p->d / p->pix;
+    const int e_max = (int)std::ceil(inv_max + 0.5) - 1;
+    const int win = round_up((int)std::ceil(127.0 * inv_max) + 2 * e_max + 8, 4);
+    const int pad = std::max(round_up(2 * e_max + 2, 4), round_up((win - p->N + 1) / 2 + 1, 4));
+    const int pitch = round_up(p->N + 2 * pad, 4);
+    // lines per staged block: as many (<= 16) as keep two stages within 48 KB, so that several CTAs share an SM
+    int lb = 16;
+    while (lb > 1 && 2 * (size_t)lb * 2 * win * p->esize > 48 * 1024) lb /= 2;
+    const size_t proj_smem = 32 + 128 + 2 * (size_t)lb * 2 * win * p->esize;
+    if (proj_smem > (size_t)kMaxDynSmem) return fail(p, FBP_EUNSUPPORTED, "fbp_project: det_spacing / pixel_size too large for the staged windows");
+    const size_t plane = (size_t)p->N * pitch;
+    if (!p->d_xt) FBP_CUDA(p, cudaMalloc(&p->d_xt, p->esize * 4 * (size_t)p->max_batch * plane));   // two copies of pairs
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    fbp::ProjParams prm{p->K, p->D, p->N, pad, 0.5 * (p->N - 1), 0.5 * (p->D - 1)};
+    fbp::ProjParams prm{p->K, p->D, p->N, pad, pitch, win, lb, 0.5 * (p->N - 1), 0.5 * (p->D - 1)};
     const dim3 tgrid((p->N + 31) / 32, (p->N + 31) / 32, batch), tblock(32, 8);
     // a thread owns a bin and its mirror bin; (bin block, angle) pairs are folded into grid.x (K may exceed 65535)
     const int bin_blocks = ((p->D + 1) / 2 + 127) / 128;
     if ((long long)bin_blocks * p->K > 0x7fffffffLL) return fail(p, FBP_EUNSUPPORTED, "n_det x n_angles too large for fbp_project");
     const dim3 pgrid((unsigned)(bin_blocks * p->K), 1, batch);
+    const size_t copy = (size_t)p->max_batch * plane;
     if (p->dtype == FBP_F32) {
-        float* xp = static_cast<float*>(p->d_xt);
-        float* xtp = xp + (size_t)p->max_batch * plane;
-        fbp::stage_image_kernel<float><<<tgrid, tblock, 0, s>>>(static_cast<const float*>(d_image), xp, xtp, p->N, pad);
-        fbp::project_kernel<float><<<pgrid, 128, 0, s>>>(xp, xtp, static_cast<float*>(d_sino), p->d_cs2, prm, bin_blocks);
+        float2* xi = static_cast<float2*>(p->d_xt);
+        static bool smem_open[kMaxDevices] = {};
+        if (cudaError_t e0 = allow_max_smem(fbp::project_kernel<float>, smem_open, p->device); e0 != cudaSuccess) return cuda_fail(p, e0, "projector setup");
+        fbp::stage_image_kernel<float><<<tgrid, tblock, 0, s>>>(static_cast<const float*>(d_image), xi, xi + copy, p->N, pad, pitch);
+        fbp::project_kernel<float><<<pgrid, 160, proj_smem, s>>>(xi, xi + copy, static_cast<float*>(d_sino), p->d_cs2, prm, bin_blocks);
     } else {
-        double* xp = static_cast<double*>(p->d_xt);
-        double* xtp = xp + (size_t)p->max_batch * plane;
-        fbp::stage_image_kernel<double><<<tgrid, tblock, 0, s>>>(static_cast<const double*>(d_image), xp, xtp, p->N, pad);
-        fbp::project_kernel<double><<<pgrid, 128, 0, s>>>(xp, xtp, static_cast<double*>(d_sino), p->d_cs2, prm, bin_blocks);
+        double2* xi = static_cast<double2*>(p->d_xt);
+        static bool smem_open[kMaxDevices] = {};
+        if (cudaError_t e0 = allow_max_smem(fbp::project_kernel<double>, smem_open, p->device); e0 != cudaSuccess) return cuda_fail(p, e0, "projector setup");
+        fbp::stage_image_kernel<double><<<tgrid, tblock, 0, s>>>(static_cast<const double*>(d_image), xi, xi + copy, p->N, pad, pitch);
+        fbp::project_kernel<double><<<pgrid, 160, proj_smem, s>>>(xi, xi + copy, static_cast<double*>(d_sino), p->d_cs2, prm, bin_blocks);
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(p, e, "projector launch");
