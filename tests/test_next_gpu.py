@@ -266,6 +266,8 @@ PROJ_CASES = [  # (N, K, D, d, pix, angle kind, batch)
     (50, 16, 40, 1.0, 1.0, "full", 1),            # detector shorter than the image: pixels fall off it
     (96, 12, 150, 0.7, 1.3, "random", 1),         # pixel > bin
     (256, 8, 363, 1.0, None, "axes", 1),          # exactly 0, pi/2, pi, ... : cos or sin = 0 and both majors
+    (48, 7, 300, 3.0, 1.0, "random", 1),          # bins 3 pixels wide: wide windows, short staged blocks, 2 bin blocks
+    (200, 5, 1100, 0.25, 1.0, "random", 1),       # pixels 4 bins wide: 5 bin blocks, most of them off the image
 ]
 
 
