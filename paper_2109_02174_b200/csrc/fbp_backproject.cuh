@@ -286,7 +286,7 @@ backproject_kernel(const uint4* __restrict__ E, T* __restrict__ image, const dou
                 }
             } else if (walk_flag[st] != 0) {
                 // walk: `near` of pixel r is the previous pixel's near (same interval) or far (next interval)
-#pragma unroll 2
+#pragma unroll 4
                 for (int a = wa; a < na; a += WA) {
                     const AngleRec<T> rc = rk[a];
                     const unsigned rowbase = segk + (unsigned)(a * L * 16);
