@@ -49,6 +49,21 @@ def main() -> int:
                     if not torch.equal(host_out, first.cpu()):
                         print("HOST MISMATCH", n, k, d, b, dt, env)
                         return 1
+                    # the forward projector (TMA-staged gather) and the cone-beam path on the same plan
+                    y1 = plan.project(first).clone()
+                    y2 = plan.project(first)
+                    torch.cuda.synchronize()
+                    if not torch.equal(y1, y2):
+                        print("PROJECT MISMATCH", n, k, d, b, dt, env)
+                        return 1
+                    if b == 1:
+                        proj = torch.from_numpy(np.random.default_rng(7).standard_normal((k, 5, d))).to(tdt).cuda()
+                        v1 = plan.fdk_reconstruct(proj, 4.0 * n, 6).clone()
+                        v2 = plan.fdk_reconstruct(proj, 4.0 * n, 6)
+                        torch.cuda.synchronize()
+                        if not torch.equal(v1, v2):
+                            print("FDK MISMATCH", n, k, d, b, dt, env)
+                            return 1
     print("selfcheck ok")
     return 0
 
@@ -82,6 +97,19 @@ def soak(runs: int) -> int:
                     if i % 25 == 0 or i == runs - 1:
                         miss += int(not torch.equal(out, first))
                 torch.cuda.synchronize()
+                if cid == 3 and not env:
+                    # the forward projector: mbarrier ring fed by a producer warp, consumers in four warps
+                    y0 = plan.project(first).clone()
+                    pmiss = 0
+                    for i in range(runs):
+                        if i % 7 == 0:
+                            junk = (junk @ junk) * 1e-4
+                        y = plan.project(first)
+                        if i % 25 == 0 or i == runs - 1:
+                            pmiss += int(not torch.equal(y, y0))
+                    torch.cuda.synchronize()
+                    print("cfg%d %s forward projector: %d runs, %d mismatches" % (cid, dt, runs, pmiss))
+                    bad += pmiss
             print("cfg%d %s batch %d %s: %d runs, %d mismatches" % (cid, dt, batch, env, runs, miss))
             bad += miss
     return 1 if bad else 0
