@@ -9,7 +9,8 @@
 // Back-projection is a gather with one owner thread per voxel column and a fixed angle order: deterministic, no
 // atomics (the paper's parallel versions were not).  For a fixed (x, y, angle) the detector column
 // and the weight do not depend on z and the detector row is affine in z: a thread owns ZT voxels of one (x, y)
-// column and pays the per-angle work once for all of them.
+// column and pays the per-angle work once for all of them.  Between 2 and 3 the filtered projections are re-packed
+// into zero-bordered 2 x 2 quads (fdk_quads_kernel) so that a bilinear sample is one aligned load without bounds tests.
 #pragma once
 #include <cuda_runtime.h>
 

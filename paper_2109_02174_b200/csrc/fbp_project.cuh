@@ -14,10 +14,11 @@
 // short run of pixels with |u - j| < 1 around p* = the position where u = j: p* is affine in the line
 // index and is evaluated in fp64 (so fp32 weights see only the small offset p - p*, never a
 // coordinate of size N); the run is round(p*) + e, |e| <= E, with E = ceil(d/(pix max(|cos|,|sin|)) + 1/2) - 1.
-// Lanes are consecutive bins, hence consecutive-ish pixels of the same line: coalesced reads.  The image
-// is first staged (stage_image_kernel) into a copy with zero columns on both sides of every line and, for
-// y-major angles, a transposed copy of the same form (roles of cos and sin swapped), so that the inner loop
-// has no bounds checks and no divergence; each thread visits only the lines its ray can touch.
+// Lanes are consecutive bins, hence consecutive-ish pixels of the same line.  The image is first staged
+// (stage_image_kernel) into zero-padded lines of (pixel, mirror pixel) pairs and, for y-major angles, a
+// transposed copy of the same form (roles of cos and sin swapped); the projector moves each line's window
+// of a CTA's bins into shared memory with one TMA bulk copy and gathers from there (see project_kernel):
+// no bounds checks, and each thread visits only the lines its ray can touch.
 #pragma once
 #include <cuda_runtime.h>
 
