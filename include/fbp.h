@@ -157,6 +157,44 @@ fbp_status fbp_metrics(fbp_plan *plan, const void *d_x, const void *d_y, long lo
                        double c1, double c2, double *d_out8, void *cuda_stream);
 
 /*
+ * fbp_metrics_static -- fbp_metrics for callers that must not allocate device memory: no plan, no cudaMalloc,
+ * no cudaFree, no allocating library routine, on any call.  Same definition (eq. 3 and 4), same
+ * kernel, same grid rule and summation order as fbp_metrics, hence the same eight outputs for the same inputs.
+ *
+ * Who needs it.  Every other compute entry point takes a plan, and fbp_create allocates.  That rules the
+ * library out for a caller that gave ALL device memory to its own pool or caching allocator at start-up (a
+ * cudaMalloc from underneath such a pool fails, or takes memory the pool believes it owns), for a loop with a
+ * latency bound (cudaMalloc / cudaFree wait for the whole device to go idle), and for a process that must account
+ * for every device byte before it starts.  Those callers compare two reconstructions with this call instead: they
+ * pass the two arrays and the result buffer, and the kernel's work area (one 48-byte partial-sum record per CTA and
+ * the finish ticket) is a fixed array inside the library image instead of plan-owned memory.
+ *
+ * The price, and the limits:
+ *   - The work area is FBP_METRICS_STATIC_MAX_CTAS (1536) records + one 256-byte line = 73 984 bytes of device
+ *     memory, held by EVERY GPU on which the library's device code gets loaded, from that moment until the
+ *     process exits, whether or not this call is ever made there.
+ *   - n <= FBP_METRICS_STATIC_MAX_N (2^31 elements per array).  A larger n is refused with FBP_EINVAL and a message
+ *     naming the limit (fbp_last_error(NULL)); nothing is enqueued.  fbp_metrics on a plan has no such limit.
+ *   - It runs on the CURRENT device (the one d_x, d_y and d_out8 belong to) and never switches devices.
+ *   - First call on each device: the library looks up where the work area sits on that device and how many CTAs
+ *     fit one wave (two occupancy queries), under a mutex, and keeps the answers.  That first call may also be what
+ *     makes the CUDA runtime load the library's device code.  Make it once per device during start-up, BEFORE any
+ *     stream capture begins on that device; later calls only enqueue a 4-byte memset and one kernel.
+ *   - All calls on a device share the one work area, and it keeps the previous call's contents (the call clears the
+ *     one word that has to start at zero).  Two calls may therefore not overlap on the GPU: issue them on one
+ *     stream, or order them with events.  Calls on different streams with nothing between them race on the
+ *     records and the ticket and return garbage without any error.  Plans are not affected (they own their scratch).
+ * Arguments as fbp_metrics, with `dtype` in place of the plan: d_x, d_y DEVICE arrays of n elements of `dtype`
+ * (aligned to the element size; 16-byte alignment takes the vector path), d_out8 DEVICE array of 8 doubles written
+ * on the stream.  Errors: FBP_EINVAL (arguments, n beyond the limit), FBP_EUNSUPPORTED (not a compute-capability-10
+ * device, or a device ordinal >= 64), FBP_ECUDA; text through fbp_last_error(NULL) on the calling thread.
+ */
+#define FBP_METRICS_STATIC_MAX_N (1LL << 31)
+#define FBP_METRICS_STATIC_MAX_CTAS 1536
+fbp_status fbp_metrics_static(fbp_dtype dtype, const void *d_x, const void *d_y, long long n, double max_val,
+                              double c1, double c2, double *d_out8, void *cuda_stream);
+
+/*
  * fbp_set_window -- choose the reconstruction filter H of PAPER.md:61 ("Q = P * H"; the paper names
  * no particular H).  The taps are the inverse DTFT of |f| W(f) on |f| <= 1/2 cycles per sample,
  *   h_W[m] = 2 * integral_0^{1/2} f W(f) cos(2 pi f m) df   (closed forms, computed in fp64 on the host):
@@ -235,7 +273,8 @@ void fbp_destroy(fbp_plan *plan);
 
 /*
  * fbp_last_error -- text of the last error on this plan (plan-owned, never freed by the
- * caller; "" if none).  NULL plan: the last fbp_create error of the calling thread.
+ * caller; "" if none).  NULL plan: the last error, on the calling thread, of the calls that take no plan
+ * (fbp_create, fbp_create_tuned, fbp_metrics_static).
  */
 const char *fbp_last_error(const fbp_plan *plan);
 

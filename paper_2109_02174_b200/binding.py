@@ -19,6 +19,7 @@ EXPORTS = (
     "fbp_create", "fbp_create_tuned", "fbp_filter", "fbp_backproject", "fbp_reconstruct", "fbp_reconstruct_host",
     "fbp_destroy", "fbp_last_error", "fbp_plan_info", "fbp_set_profiling", "fbp_get_kernel_ms",
     "fbp_set_trace", "fbp_metrics", "fbp_set_window", "fbp_set_angle_weights", "fbp_interpolate_stack", "fbp_project", "fbp_fdk_reconstruct",
+    "fbp_metrics_static",
 )
 
 PLAN_INFO_FIELDS = (
@@ -67,6 +68,8 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         fn.restype = ci
     lib.fbp_metrics.argtypes = [vp, vp, vp, ctypes.c_longlong, cd, cd, cd, vp, vp]
     lib.fbp_metrics.restype = ci
+    lib.fbp_metrics_static.argtypes = [ci, vp, vp, ctypes.c_longlong, cd, cd, cd, vp, vp]
+    lib.fbp_metrics_static.restype = ci
     lib.fbp_set_window.argtypes = [vp, ci]
     lib.fbp_set_window.restype = ci
     lib.fbp_set_angle_weights.argtypes = [vp, ctypes.POINTER(cd)]
@@ -215,6 +218,24 @@ def fbp_metrics(plan, d_x, d_y, n, max_val, c1, c2, d_out8, stream=None):
     lib = load_library()
     _check(lib, plan, lib.fbp_metrics(plan, _ptr(d_x), _ptr(d_y), int(n), float(max_val), float(c1), float(c2),
                                       _ptr(d_out8), _stream_handle(stream)))
+
+
+METRICS_STATIC_MAX_N = 1 << 31   # FBP_METRICS_STATIC_MAX_N of include/fbp.h
+
+
+def fbp_metrics_static(dtype, d_x, d_y, n, max_val, c1, c2, d_out8, stream=None):
+    """fbp_metrics_static of include/fbp.h: PSNR / SSIM of two device arrays with no plan and no device allocation.
+
+    For programs that cannot let this library call cudaMalloc (all device memory already owned by their own pool,
+    a latency-bound loop, a fixed memory budget): the kernel's work area is a fixed 73 984-byte array inside
+    libfbp.so instead of plan-owned memory.  The caller passes every buffer, `d_out8` (8 doubles on the device)
+    included, so this wrapper allocates nothing either.  `dtype` is FBP_F32 or FBP_F64; the current CUDA device
+    must be the one the arrays live on.  n > METRICS_STATIC_MAX_N raises FbpError(FBP_EINVAL).  Calls share the
+    work area: keep them on one stream (or order them with events), and make the first call on each device
+    during start-up, before any stream capture."""
+    lib = load_library()
+    _check(lib, None, lib.fbp_metrics_static(int(dtype), _ptr(d_x), _ptr(d_y), int(n), float(max_val), float(c1),
+                                             float(c2), _ptr(d_out8), _stream_handle(stream)))
 
 
 WINDOWS = {"ramlak": 0, "shepp-logan": 1, "cosine": 2, "hamming": 3, "hann": 4}

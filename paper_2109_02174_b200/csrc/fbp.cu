@@ -1305,3 +1305,131 @@ fbp_status fbp_get_kernel_ms(fbp_plan* p, float* filter_ms, float* backproject_m
 }
 
 }  // extern "C"
+
+// ---- fbp_metrics_static: the metrics reduction for callers that may not allocate -----------------------------
+// fbp_metrics needs a plan, and making a plan calls cudaMalloc.  Some users of this library never get to do
+// that: a process whose device memory was handed, all of it, to a pool or caching allocator at start-up (a
+// cudaMalloc from a library underneath it fails or eats into what the pool counts as its own); a control loop
+// with a latency bound (cudaMalloc and cudaFree wait for the whole device); a process held to a fixed memory
+// budget in which every allocation is accounted for up front.  For them the CTA partial sums and the finish
+// ticket of metrics_kernel live in the array below, which is part of the library image: the driver places it
+// when the library's device code is loaded on a GPU, and it stays there, on every GPU that loads the library,
+// until the process exits.  Size: 1536 CTA records of six doubles + one 256-byte line for the ticket = 73 984
+// bytes.
+//
+// `g_metrics_static_scratch` is a device symbol.  Device code may name it; in HOST code the name is only a
+// stand-in handle for the runtime -- not a device address -- so nothing below ever hands `g_metrics_static_scratch`
+// itself to a kernel: the address is asked for once per device with cudaGetSymbolAddress, with that device
+// current, and the pointer it returns is what the kernel gets.
+namespace {
+constexpr int kStaticMetricCtas = kMetricGridMax;                              // CTA records the array holds
+constexpr int kStaticTicketAt = fbp::kMetricSums * kStaticMetricCtas;          // in doubles: byte 73 728, a multiple of 256
+constexpr long long kStaticMetricMaxN = 1LL << 31;                             // FBP_METRICS_STATIC_MAX_N of fbp.h
+static_assert(kStaticMetricMaxN == FBP_METRICS_STATIC_MAX_N, "fbp.h and fbp.cu disagree on the limit");
+static_assert(kStaticMetricCtas == FBP_METRICS_STATIC_MAX_CTAS, "fbp.h and fbp.cu disagree on the scratch size");
+static_assert((kStaticTicketAt * sizeof(double)) % 256 == 0, "the ticket sits on its own 256-byte line");
+}  // namespace
+
+static __device__ __align__(256) double g_metrics_static_scratch[kStaticTicketAt + 256 / sizeof(double)];
+
+namespace {
+
+struct StaticMetricsDevice {
+    bool ready = false;
+    double* scratch = nullptr;     // device address of g_metrics_static_scratch ON THIS DEVICE
+    int grid_max[2] = {0, 0};      // one wave of metrics_kernel<float> / <double>, as launch_metrics sizes it
+};
+StaticMetricsDevice g_static_metrics[kMaxDevices];
+std::mutex g_static_metrics_mutex;
+
+// Once per device, with that device current (the caller's: this entry point never switches devices).
+fbp_status static_metrics_setup(int device, StaticMetricsDevice& out)
+{
+    std::lock_guard<std::mutex> lock(g_static_metrics_mutex);
+    StaticMetricsDevice& sd = g_static_metrics[device];
+    if (!sd.ready) {
+        int major = 0, sms = 0;
+        cudaError_t e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device);
+        if (e != cudaSuccess) return cuda_fail(nullptr, e, "fbp_metrics_static: cudaDeviceGetAttribute");
+        if (major != 10)
+            return fail(nullptr, FBP_EUNSUPPORTED, "libfbp is built for sm_100a (B200) only; no fallback path");
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
+        if (e != cudaSuccess) return cuda_fail(nullptr, e, "fbp_metrics_static: cudaDeviceGetAttribute");
+        if (sms < 1) sms = 148;
+        int per_sm[2] = {0, 0};
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[0], fbp::metrics_kernel<float>, fbp::kMetricThreads, 0);
+        if (e != cudaSuccess) return cuda_fail(nullptr, e, "fbp_metrics_static: occupancy query");
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[1], fbp::metrics_kernel<double>, fbp::kMetricThreads, 0);
+        if (e != cudaSuccess) return cuda_fail(nullptr, e, "fbp_metrics_static: occupancy query");
+        double* ptr = nullptr;
+        e = cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), g_metrics_static_scratch);
+        if (e != cudaSuccess) return cuda_fail(nullptr, e, "fbp_metrics_static: cudaGetSymbolAddress");
+        if (!ptr) return fail(nullptr, FBP_ECUDA, "fbp_metrics_static: cudaGetSymbolAddress returned no address");
+        sd.scratch = ptr;
+        for (int t = 0; t < 2; ++t) sd.grid_max[t] = std::min(std::max(per_sm[t], 1) * sms, kStaticMetricCtas);
+        sd.ready = true;
+    }
+    out = sd;
+    return FBP_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+fbp_status fbp_metrics_static(fbp_dtype dtype, const void* d_x, const void* d_y, long long n, double max_val,
+                              double c1, double c2, double* d_out8, void* stream)
+{
+    if (dtype != FBP_F32 && dtype != FBP_F64) return fail(nullptr, FBP_EINVAL, "fbp_metrics_static: unknown dtype");
+    if (!d_x || !d_y || !d_out8) return fail(nullptr, FBP_EINVAL, "fbp_metrics_static: NULL device pointer");
+    if (n < 1) return fail(nullptr, FBP_EINVAL, "fbp_metrics_static: n must be >= 1");
+    if (n > kStaticMetricMaxN) {
+        char msg[200];
+        std::snprintf(msg, sizeof msg, "fbp_metrics_static: n = %lld exceeds FBP_METRICS_STATIC_MAX_N = %lld elements; "
+                      "use fbp_metrics on a plan for larger inputs", n, kStaticMetricMaxN);
+        return fail(nullptr, FBP_EINVAL, msg);
+    }
+    if (!(max_val > 0.0) || !std::isfinite(max_val))
+        return fail(nullptr, FBP_EINVAL, "fbp_metrics_static: max_val must be finite and > 0");
+    if ((reinterpret_cast<uintptr_t>(d_out8) & 7u) != 0)
+        return fail(nullptr, FBP_EINVAL, "fbp_metrics_static: d_out8 must be 8-byte aligned");
+    const size_t esize = dtype == FBP_F32 ? 4 : 8;
+    if ((reinterpret_cast<uintptr_t>(d_x) | reinterpret_cast<uintptr_t>(d_y)) & (esize - 1))
+        return fail(nullptr, FBP_EINVAL, "fbp_metrics_static: d_x and d_y must be aligned to the element size");
+    if (c1 < 0.0) c1 = (0.01 * max_val) * (0.01 * max_val);
+    if (c2 < 0.0) c2 = (0.03 * max_val) * (0.03 * max_val);
+
+    int device = -1;
+    cudaError_t e = cudaGetDevice(&device);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "fbp_metrics_static: cudaGetDevice");
+    if (device < 0 || device >= kMaxDevices)
+        return fail(nullptr, FBP_EUNSUPPORTED, "fbp_metrics_static: device ordinal beyond the 64 this entry point keeps state for");
+    StaticMetricsDevice sd;
+    fbp_status st = static_metrics_setup(device, sd);
+    if (st != FBP_OK) return st;
+
+    // the same grid rule as launch_metrics, so the sums are added in the same order as on a plan
+    const int t = dtype == FBP_F32 ? 0 : 1;
+    const long long want = (n + 32LL * fbp::kMetricThreads - 1) / (32LL * fbp::kMetricThreads);
+    const int grid = (int)(want < sd.grid_max[t] ? want : sd.grid_max[t]);
+    double* partial = sd.scratch;
+    unsigned* ticket = reinterpret_cast<unsigned*>(sd.scratch + kStaticTicketAt);
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    // The array is shared by every call and keeps what the last one left.  Partials: each CTA of this launch
+    // overwrites its own record before anyone reads it, records of a larger earlier grid are never read.  The
+    // ticket must be 0 when the kernel starts; the kernel re-arms it as it finishes, but a launch that died
+    // half-way would leave it counting, so it is cleared here, on the caller's stream, every time.
+    e = cudaMemsetAsync(ticket, 0, sizeof(unsigned), s);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "fbp_metrics_static: clearing the ticket");
+    if (dtype == FBP_F32)
+        fbp::metrics_kernel<float><<<grid, fbp::kMetricThreads, 0, s>>>(static_cast<const float*>(d_x), static_cast<const float*>(d_y),
+                                                                        n, partial, ticket, max_val, c1, c2, d_out8);
+    else
+        fbp::metrics_kernel<double><<<grid, fbp::kMetricThreads, 0, s>>>(static_cast<const double*>(d_x), static_cast<const double*>(d_y),
+                                                                         n, partial, ticket, max_val, c1, c2, d_out8);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "fbp_metrics_static: launch");
+    return FBP_OK;
+}
+
+}  // extern "C"
