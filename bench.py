@@ -56,6 +56,8 @@ def parse_args():
                     help="launch-configuration override passed to fbp_create_tuned (A/B runs), e.g. --opt filter_kind=1")
     ap.add_argument("--graph", action="store_true",
                     help="also time the step replayed as ONE CUDA graph (the two launches with their programmatic edge captured once)")
+    ap.add_argument("--lib", default=None, metavar="PATH",
+                    help="load this build of libfbp.so instead of the in-tree one (A/B of two builds; recorded in launch.lib)")
     ap.add_argument("--extras", action="store_true", help="also time fbp_metrics, fbp_interpolate_stack and fbp_project")
     return ap.parse_args()
 
@@ -495,7 +497,7 @@ def main():
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    fbp.load_library()
+    fbp.load_library(args.lib)
 
     r = measure(args, args.dtype, world, rank, local, dist)
     r64 = None

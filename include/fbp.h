@@ -80,7 +80,8 @@ fbp_status fbp_create(fbp_plan **out, int n_angles, int n_det, const double *ang
  * bits of a result), never the definition of what is computed; each plan stays bit-reproducible.
  *   FBP_OPT_BP_VARIANT      index of the back-projection tile variant (R rows/thread, warps in y, angle groups)
  *   FBP_OPT_BP_SPLITS       angle splits S per tile (>= 1)        FBP_OPT_BP_CHUNK   angles staged per chunk (<= 32)
- *   FBP_OPT_FILTER_R        output pairs per thread of the direct-form filter (6, 10, 14; dense 5, 7, 9)
+ *   FBP_OPT_FILTER_R        output pairs per thread of the direct-form filter (6, 10, 14; dense 5, 7, 9; fp64 plans: 6 or 5
+ *                           only); any other value, or one the plan's dtype does not have, is FBP_EINVAL
  *   FBP_OPT_FILTER_SB       warps (input slices) per filter CTA (1..8)
  *   FBP_OPT_FILTER_KIND     0 = library's choice, 1 = direct form, 2 = FFT form
  *   FBP_OPT_PIPELINE        0 = no batch pipeline; FBP_OPT_PIPE_GROUP slices per pipeline group;
@@ -251,8 +252,10 @@ fbp_status fbp_project(fbp_plan *plan, const void *d_image, void *d_sino, int ba
  *                    t = x cos + y sin,  U = sad - x sin + y cos,  zero outside the detector.
  * d_proj [K][n_rows][n_det] in, d_volume [n_z][N][N] out (DEVICE, plan dtype, 16-byte aligned).  sad must exceed the
  * image's half-diagonal (FBP_EINVAL otherwise).  The first call (and any call with more rows than before) allocates
- * plan-owned scratch (synchronous); later calls only enqueue.  One owner thread per voxel, fixed order: deterministic.
- * Angle weights do not apply.
+ * plan-owned scratch (synchronous); later calls only enqueue.  That scratch is about SIX times the projection set --
+ * the weighted copy, the filtered copy and the zero-bordered 2 x 2 quads, 4 (n_rows + 2)(n_det + 2) K elements -- and
+ * is kept until fbp_destroy.  A projection set of more than 2^31 x 256 elements is FBP_EINVAL.  One owner thread per
+ * voxel, fixed order: deterministic.  Angle weights do not apply.
  */
 fbp_status fbp_fdk_reconstruct(fbp_plan *plan, const void *d_proj, void *d_volume, int n_rows, double row_spacing,
                                double sad, int n_z, double voxel_z, void *cuda_stream);
@@ -300,14 +303,20 @@ int fbp_plan_info(const fbp_plan *plan, int *out, int n);
  * fbp_set_trace -- optional in-kernel timeline (profiles/: where the microseconds of a step go).  d_marks: DEVICE
  * array of `capacity` 64-bit words (caller-owned, zero it first), or NULL to switch tracing off.  While set, thread 0
  * of every CTA of the filter and of the back-projector stores %globaltimer (ns) into its 8-word record:
- *   filter CTA c          -> d_marks[8 c + s],  s = 0 start, 1 tables and first row staged, 2 partial sums done,
- *                            3 row reduced, 4 last unit stored (1-3: the CTA's first unit only)
+ *   filter CTA c          -> d_marks[8 c + s],  direct form: s = 0 start, 1 tables and first row staged, 2 partial sums
+ *                            done, 3 row reduced, 4 last unit stored (1-3: the CTA's first unit only);
+ *                            FFT form: s = 0 start, 1 row pair read and first pass done, 2 spectrum ready (forward passes
+ *                            done, before the product with the kernel's DFT), 3 rows back in shared memory (inverse
+ *                            passes done), 4 last row pair stored (1-3: the CTA's first row pair only)
  *   back-projector CTA c  -> d_marks[8 (F + c) + s],  F = plan_info[16],  s = 0 CTA resident, 1 past the grid
  *                            dependency, 2 first chunk landed, 3 main loop done, 4 pixels stored,
  *                            7 the SM the CTA ran on (%smid, not a time)
  * A kernel whose records would not fit in `capacity` is not traced.  The filters carry the marks as predicated
  * stores; the back-projector runs a second instantiation of the same source with the marks compiled in (under its
- * register cap even predicated-off marks cost the main loop).  Not used by the batch pipeline's side streams.
+ * register cap even predicated-off marks cost the main loop).  Traced launches are those of fbp_filter,
+ * fbp_backproject, fbp_reconstruct and fbp_reconstruct_host when they run one filter launch and one back-projector
+ * launch; the batch pipeline's per-group launches (which would overwrite each other's records) and the launches of
+ * fbp_fdk_reconstruct (whose filter grid is sized for K x n_rows rows) never write marks.
  */
 fbp_status fbp_set_trace(fbp_plan *plan, unsigned long long *d_marks, long long capacity);
 

@@ -39,6 +39,8 @@ class Plan:
         self.torch_dtype = torch.float32 if _DTYPES[dtype] == FBP_F32 else torch.float64
         self.n_angles, self.n_det, self.image_n, self.max_batch = len(angles_rad), int(n_det), int(image_n), int(max_batch)
         self.device = torch.device("cuda", torch.cuda.current_device() if device < 0 else device)
+        # pixel size as the C side resolves it (fbp_create: pixel_size <= 0 means "= det_spacing")
+        self.pixel_size = float(pixel_size) if pixel_size > 0 else float(det_spacing)
         if options:
             self.handle = fbp_create_tuned(self.n_angles, n_det, angles_rad, det_spacing, image_n, pixel_size,
                                            _DTYPES[dtype], max_batch, device, options)
@@ -111,7 +113,8 @@ class Plan:
         return out
 
     def fdk_reconstruct(self, proj, sad, n_z, row_spacing=1.0, voxel_z=None, out=None, stream=None):
-        """Cone-beam FDK: projections [K][n_rows][n_det] -> volume [n_z][N][N] (include/fbp.h, fbp_fdk_reconstruct)."""
+        """Cone-beam FDK: projections [K][n_rows][n_det] -> volume [n_z][N][N] (include/fbp.h, fbp_fdk_reconstruct).
+        voxel_z=None means isotropic voxels: the plan's pixel size (not the detector's row spacing)."""
         import torch
         if (proj.dtype != self.torch_dtype or not proj.is_cuda or not proj.is_contiguous() or proj.dim() != 3
                 or proj.shape[0] != self.n_angles or proj.shape[2] != self.n_det):
@@ -123,7 +126,7 @@ class Plan:
               or out.device != proj.device):
             raise ValueError("out must be a contiguous CUDA tensor [n_z][N][N] of the plan dtype")
         fbp_fdk_reconstruct(self.handle, proj, out, proj.shape[1], row_spacing, sad, n_z,
-                            row_spacing if voxel_z is None else voxel_z, stream)
+                            self.pixel_size if voxel_z is None else voxel_z, stream)
         return out
 
     def set_window(self, window):

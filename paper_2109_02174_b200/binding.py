@@ -50,7 +50,7 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     global _lib
     if _lib is not None and path is None:
         return _lib
-    path = path or os.environ.get("FBP_LIB") or _build.LIB   # FBP_LIB: A/B builds of the same library
+    path = path or _build.LIB          # an A/B build of the library is loaded by passing its path: nothing else picks the file
     if not os.path.exists(path):
         raise FileNotFoundError(
             "%s not found: build it with `python -m paper_2109_02174_b200.build` "

@@ -97,6 +97,9 @@ struct fbp_plan {
     cudaEvent_t ev_fork = nullptr, ev_f[kMaxGroups] = {}, ev_b[2] = {nullptr, nullptr};
     unsigned long long* d_trace = nullptr;   // fbp_set_trace (caller-owned)
     long long trace_cap = 0;
+    bool trace_launch = false;               // set by run_filter / run_bp around their own launch only: the batch pipeline's
+                                             // groups and the cone-beam path's K x n_rows filter launch would overwrite or overrun
+                                             // the records (include/fbp.h: "fbp_filter, fbp_backproject, fbp_reconstruct only")
     bool profiling = false;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     bool ran_filter = false, ran_bp = false;
@@ -138,6 +141,14 @@ struct DeviceGuard {
 };
 
 int round_up(int v, int m) { return (v + m - 1) / m * m; }
+
+// The trace buffer as THIS launch sees it: NULL unless tracing is on and the launch comes from run_filter / run_bp.
+unsigned long long* trace_of(const fbp_plan* p) { return p->trace_launch ? p->d_trace : nullptr; }
+struct TraceScope {
+    fbp_plan* p;
+    explicit TraceScope(fbp_plan* plan) : p(plan) { p->trace_launch = true; }
+    ~TraceScope() { p->trace_launch = false; }
+};
 
 // The dynamic shared-memory limit is an attribute of the KERNEL (per context), not of a plan: plans with
 // different geometries share the instantiations, so each one is opened up once per device to the device
@@ -499,7 +510,7 @@ cudaError_t launch_filter3_r(fbp_plan* p, const void* sino, void* filt, void* en
     // persistent: never more CTAs than are co-resident (tables staged once per CTA)
     const long long work = (long long)f.n_rows * f.n_units;
     const int grid = (int)std::min<long long>(work, c.grid_cap);
-    if (p->d_trace && 8LL * grid <= p->trace_cap) f.trace = p->d_trace;
+    if (trace_of(p) && 8LL * grid <= p->trace_cap) f.trace = trace_of(p);
     kern<<<grid, c.threads, c.smem, st>>>(static_cast<const T*>(sino), static_cast<T*>(filt), static_cast<uint4*>(ent),
                                           static_cast<const T*>(c.d_u), static_cast<const T*>(c.d_rho),
                                           static_cast<const T*>(p->d_wrow), p->K, f, (T)(1.0 / p->d));
@@ -524,7 +535,7 @@ cudaError_t launch_fft_p(fbp_plan* p, const void* sino, void* filt, void* ent, i
                      ent ? p->d_cs2 : nullptr, (int)(sizeof(double2) * (size_t)p->K), nullptr};
     const long long work = (long long)batch * f.pairs_per_slice;
     const int grid = (int)std::min<long long>(work, c.grid_cap);
-    if (p->d_trace && 8LL * grid <= p->trace_cap) f.trace = p->d_trace;
+    if (trace_of(p) && 8LL * grid <= p->trace_cap) f.trace = trace_of(p);
     kern<<<grid, c.threads, c.smem, st>>>(static_cast<const T*>(sino), static_cast<T*>(filt), static_cast<uint4*>(ent),
                                           static_cast<const fbp::Cx<T>*>(c.d_tab), static_cast<const T*>(p->d_wrow), f);
     return cudaGetLastError();
@@ -616,7 +627,7 @@ cudaError_t launch_bp_t(fbp_plan* p, void* image, int batch, cudaStream_t st, in
     fbp::BpParams prm = p->bp;
     // trace records of the back-projector follow the filter's (fbp_set_trace)
     prm.trace = nullptr;
-    if (p->d_trace) {
+    if (trace_of(p)) {
         const long long f_ctas = filter_ctas(p);   // plan_info[16]
         const long long b_ctas = (long long)cfg.gridDim.x * cfg.gridDim.y * cfg.gridDim.z;
         if (8 * (f_ctas + b_ctas) <= p->trace_cap) prm.trace = p->d_trace + 8 * f_ctas;
@@ -628,7 +639,7 @@ cudaError_t launch_bp_t(fbp_plan* p, void* image, int batch, cudaStream_t st, in
 template <typename T, int R, int WY, int WA>
 cudaError_t launch_bp_v(fbp_plan* p, void* image, int batch, cudaStream_t st, int slice0)
 {
-    return p->d_trace ? launch_bp_t<T, R, WY, WA, true>(p, image, batch, st, slice0)
+    return trace_of(p) ? launch_bp_t<T, R, WY, WA, true>(p, image, batch, st, slice0)
                       : launch_bp_t<T, R, WY, WA, false>(p, image, batch, st, slice0);
 }
 
@@ -665,6 +676,7 @@ fbp_status check_call(fbp_plan* p, const void* a, const void* b, int batch)
 fbp_status run_filter(fbp_plan* p, const void* sino, void* filt, void* ent, int batch, cudaStream_t st)
 {
     if (p->profiling) FBP_CUDA(p, cudaEventRecord(p->ev[0], st));
+    TraceScope traced(p);
     cudaError_t e = p->dtype == FBP_F32 ? launch_filter<float>(p, sino, filt, ent, batch, st)
                                         : launch_filter<double>(p, sino, filt, ent, batch, st);
     if (e != cudaSuccess) return cuda_fail(p, e, "filter launch");
@@ -683,6 +695,7 @@ fbp_status run_bp(fbp_plan* p, const void* filt, void* image, int batch, cudaStr
         if (e != cudaSuccess) return cuda_fail(p, e, "entries launch");
     }
     if (p->profiling) FBP_CUDA(p, cudaEventRecord(p->ev[2], st));
+    TraceScope traced(p);
     e = p->dtype == FBP_F32 ? launch_bp<float>(p, image, batch, st) : launch_bp<double>(p, image, batch, st);
     if (e != cudaSuccess) return cuda_fail(p, e, "back-projection launch");
     if (p->profiling) FBP_CUDA(p, cudaEventRecord(p->ev[3], st));
@@ -769,6 +782,16 @@ fbp_status create_impl(fbp_plan** out, int n_angles, int n_det, const double* an
     if (!std::isfinite(pixel_size)) return fail(nullptr, FBP_EINVAL, "pixel_size must be finite");
     if (dtype != FBP_F32 && dtype != FBP_F64) return fail(nullptr, FBP_EINVAL, "unknown dtype");
     if (max_batch < 1 || max_batch > 65535) return fail(nullptr, FBP_EINVAL, "max_batch must be in [1, 65535]");
+    // FBP_OPT_FILTER_R names a group size of the direct-form filter: 6, 10, 14 (Ram-Lak, sparse taps) or 5, 7, 9
+    // (windowed, dense taps); fp64 plans have the smallest of each only (larger ones spill).  A value the plan
+    // cannot honour is an error, not a silent fallback to the library's choice.
+    if (tune.filter_r != 0) {
+        const int r = tune.filter_r;
+        const bool known = r == 5 || r == 6 || r == 7 || r == 9 || r == 10 || r == 14;
+        if (!known) return fail(nullptr, FBP_EINVAL, "FBP_OPT_FILTER_R must be one of 6, 10, 14 (Ram-Lak) or 5, 7, 9 (windowed)");
+        if (dtype == FBP_F64 && r != 5 && r != 6)
+            return fail(nullptr, FBP_EINVAL, "FBP_OPT_FILTER_R: fp64 plans run the direct-form filter with R = 6 (Ram-Lak) or 5 (windowed) only");
+    }
     for (int i = 0; i < n_angles; ++i)
         if (!std::isfinite(angles_rad[i])) return fail(nullptr, FBP_EINVAL, "non-finite angle");
     const double pix = pixel_size > 0.0 ? pixel_size : det_spacing;
@@ -1124,6 +1147,9 @@ fbp_status fbp_fdk_reconstruct(fbp_plan* p, const void* d_proj, void* d_volume, 
     const size_t pairs_per_angle = (size_t)(n_rows + 2) * (size_t)(p->D + 2);
     if (pairs_per_angle > 0x7fffffffULL) return fail(p, FBP_EINVAL, "detector too large");
     const size_t pairs = pairs_per_angle * p->K;
+    // the two elementwise kernels run one thread per element / quad in a one-dimensional grid
+    if ((elems + 255) / 256 > 0x7fffffffULL || (pairs + 255) / 256 > 0x7fffffffULL)
+        return fail(p, FBP_EINVAL, "projection set too large (more than 2^31 x 256 elements)");
     const size_t need = 2 * elems + 4 + 4 * pairs;   // elements: weighted | filtered | (pad to a quad) | quads
     if (need > p->fdk_elems) {                       // first call (or a taller detector): synchronous, like fbp_project
         FBP_CUDA(p, cudaDeviceSynchronize());

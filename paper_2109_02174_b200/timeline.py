@@ -14,7 +14,11 @@ import argparse
 
 import numpy as np
 
-FILTER_SLOTS = ("start", "tables+row staged", "partial sums done", "row reduced", "last unit stored")
+# slot names of include/fbp.h (fbp_set_trace), per filter kind (plan_info "filter_kind": 1 direct form, 2 FFT form)
+FILTER_SLOTS = {
+    1: ("start", "tables+row staged", "partial sums done", "row reduced", "last unit stored"),
+    2: ("start", "rows read, 1st pass", "spectrum ready", "rows back in smem", "last row pair stored"),
+}
 BP_SLOTS = ("CTA resident", "past grid dependency", "first chunk landed", "main loop done", "pixels stored")
 
 
@@ -75,7 +79,7 @@ def main() -> int:
           % (args.config, args.dtype, B, options, n_f, info["filter_threads"], info["filter_units_per_row"], n_b, info["bp_threads"]))
     print("microseconds after the first filter CTA started (median over %d repetitions, L2 mode '%s', of min / median / max over CTAs)" % (args.reps, args.l2))
     k = 0
-    for kern, slots in (("filter", FILTER_SLOTS), ("back-projection", BP_SLOTS)):
+    for kern, slots in (("filter", FILTER_SLOTS[info["filter_kind"]]), ("back-projection", BP_SLOTS)):
         for s in slots:
             print("%-16s %-22s %8.2f %8.2f %8.2f" % (kern, s, med[k], med[k + 1], med[k + 2]))
             k += 3

@@ -63,6 +63,12 @@ def test_create_tuned_rejects_bad_option_lists(lib):
     assert plan.value is None
     assert lib.fbp_create_tuned(ctypes.byref(plan), 4, 8, ang, 1.0, 8, 1.0, 0, 1, -1, None, 2) == pkg.FBP_EINVAL
     assert lib.fbp_create_tuned(ctypes.byref(plan), 4, 8, ang, 1.0, 8, 1.0, 0, 1, -1, bad_key, -1) == pkg.FBP_EINVAL
+    # FBP_OPT_FILTER_R: a group size no kernel has, or one the dtype does not have, is refused (checked before any CUDA call)
+    for dtype, r in ((0, 8), (0, -6), (1, 10), (1, 14), (1, 7)):
+        opt = (ctypes.c_int * 2)(pkg.OPTIONS["filter_r"], r)
+        plan.value = 123
+        assert lib.fbp_create_tuned(ctypes.byref(plan), 4, 8, ang, 1.0, 8, 1.0, dtype, 1, -1, opt, 1) == pkg.FBP_EINVAL, (dtype, r)
+        assert plan.value is None and "FBP_OPT_FILTER_R" in pkg.fbp_last_error(None)
     with pytest.raises(ValueError):
         pkg.fbp_create(5, 8, [0.0, 0.5, 1.0, 1.5], 1.0, 8, 0.0, pkg.FBP_F32)     # the C side would read 5 doubles
     with pytest.raises(ValueError):
@@ -75,6 +81,8 @@ def test_library_does_not_read_the_environment():
         for f in files:
             src = open(os.path.join(dirpath, f)).read()
             assert "getenv" not in src and "environ[" not in src and "putenv" not in src, f
+    binding = open(os.path.join(ROOT, "paper_2109_02174_b200", "binding.py")).read()
+    assert "environ" not in binding and "getenv" not in binding          # which .so is loaded is an argument too
 
 
 def test_null_plan_is_rejected_or_ignored(lib):

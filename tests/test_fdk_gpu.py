@@ -98,3 +98,20 @@ def test_fdk_window_and_errors(fbp, oracle):
             assert ei.value.status == fbp.FBP_EINVAL
         torch.cuda.synchronize()
         assert bool((vol == 7.0).all())
+
+
+@pytest.mark.parametrize("pixel_size", [0.5, 0.0])
+def test_fdk_default_voxel_height_is_the_pixel_size(fbp, oracle, pixel_size):
+    """voxel_z left out means isotropic voxels on both sides: the plan's pixel size (pixel_size <= 0: the detector
+    spacing, as fbp_create resolves it), whatever the detector's row spacing is."""
+    n, k, n_a, n_b, n_z, d_a, d_b, sad = 20, 18, 47, 9, 7, 0.75, 1.5, 40.0
+    ang = I.uniform_angles(k, 2 * math.pi)
+    proj = np.random.default_rng(9).normal(size=(k, n_b, n_a))
+    pix = pixel_size if pixel_size > 0 else d_a
+    ref = oracle.fdk_reconstruct(proj, ang, sad, n, n_z, d_a, d_b, pix)                 # oracle default: voxel_z = pix
+    with fbp.Plan(list(ang), n_a, n, det_spacing=d_a, pixel_size=pixel_size, dtype="f64") as plan:
+        assert plan.pixel_size == pix
+        got = plan.fdk_reconstruct(_dev(proj, "f64"), sad, n_z, row_spacing=d_b)
+    _check(got.cpu().numpy(), ref, "f64", "default voxel_z")
+    other = oracle.fdk_reconstruct(proj, ang, sad, n, n_z, d_a, d_b, pix, d_b)          # the old default would give this volume
+    assert np.abs(other - ref).max() > 1e-3 * np.abs(ref).max()

@@ -338,11 +338,19 @@ def test_filter_decompositions_match_oracle(fbp, oracle, dt, opts):
     """The direct-form row filter cuts a row into mirrored units of one warp-width (fbp_filter3.cuh): other group sizes R and other
     numbers of input slices must meet the same tolerances, on rows of 1, 2 and several units, and launching without
     programmatic dependent launch must not change a byte."""
+    if dt == "f64" and opts.get("filter_r", 6) != 6:
+        # fp64 plans have R = 6 only: the option is refused, not silently replaced by the library's choice
+        with pytest.raises(fbp.FbpError) as ei:
+            fbp.Plan(list(I.uniform_angles(9)), 70, 45, dtype=dt, options=dict(opts, filter_kind=1))
+        assert ei.value.status == fbp.FBP_EINVAL
+        return
     for n, k, dd, d in ((45, 9, 70, 0.5), (96, 7, 501, 1.0), (64, 5, 1203, 1.0)):
         sino = I.random_sinogram(31 + dd, 2, k, dd)
         ang = I.uniform_angles(k)
         sino_in = sino.astype(_np_dtype(dt))
         with fbp.Plan(list(ang), dd, n, det_spacing=d, dtype=dt, max_batch=2, options=dict(opts, filter_kind=1)) as plan:
+            if "filter_r" in opts:
+                assert plan.info()["filter_outputs_per_thread"] == 2 * opts["filter_r"]      # the R asked for is the R that runs
             ds = _to_dev(sino_in, dt)
             q = plan.filter(ds)
             f = plan.reconstruct(ds)
