@@ -376,8 +376,10 @@ def measure(args, dtype, world, rank, local, dist):
         p_ms = timed_loop(pfn, 10) / 10
         # fbp_fdk_reconstruct: cone-beam FDK of a 64-slice volume on the config's x-y grid from n_det x 97 projections
         # (pre-weight + row filter + weighted bilinear back-projection); voxel-angle updates per second of the whole call
-        n_rows, n_z, sad = 97, 64, 2.0 * N
-        d_cone = torch.empty((K, n_rows, D), dtype=tdt, device="cuda").normal_()
+        # on the seeded three-ball projections that tests/test_extras_sizes_gpu.py checks against the oracle at this size
+        # (the plan's angles span [0, pi): the timing does not depend on the angle values, the parity test uses 2 pi)
+        _, sad, n_rows, n_z = I.fdk_bench_geometry(args.config)
+        d_cone = torch.from_numpy(I.fdk_bench_projections(args.config).astype(npdt)).cuda()
         d_vol = torch.empty((n_z, N, N), dtype=tdt, device="cuda")
         kfn = lambda: fbp.fbp_fdk_reconstruct(plan.handle, d_cone, d_vol, n_rows, 1.0, sad, n_z, 1.0, stream)  # noqa: E731
         for _ in range(2):

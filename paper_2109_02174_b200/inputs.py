@@ -272,3 +272,25 @@ def ball_cone_projections(balls, angles, sad, n_a, n_b, d_a=1.0, d_b=1.0) -> np.
         dist2 = wx * wx + wy * wy + wz * wz - along * along
         out += rho * 2.0 * np.sqrt(np.maximum(rad * rad - dist2, 0.0))
     return out
+
+
+# The cone-beam workload `bench.py --extras` times and tests/test_extras_sizes_gpu.py checks against the oracle: on a
+# config's x-y grid and angle count (angles over 2 pi), 97 detector rows of the config's n_det bins, 64 slices of
+# isotropic voxels, source distance 2 N, three balls (a large central one, two small off-centre ones, one of them
+# negative) sized relative to the half-width of the image.
+FDK_BENCH_ROWS, FDK_BENCH_SLICES = 97, 64
+
+
+def fdk_bench_geometry(cfg_id: int):
+    """(angles[K] over 2 pi, sad, n_rows, n_z) of the bench's cone-beam problem on config ``cfg_id``'s grid."""
+    cfg = CONFIGS[cfg_id]
+    return uniform_angles(cfg.n_angles, 2.0 * math.pi), 2.0 * cfg.image_n, FDK_BENCH_ROWS, FDK_BENCH_SLICES
+
+
+def fdk_bench_projections(cfg_id: int) -> np.ndarray:
+    """fp64 projections [K][97][n_det] of the three-ball phantom for ``fdk_bench_geometry(cfg_id)`` (analytic)."""
+    cfg = CONFIGS[cfg_id]
+    ang, sad, n_rows, _ = fdk_bench_geometry(cfg_id)
+    h = 0.5 * cfg.image_n
+    balls = [(1.0, 0.6 * h, 0.0, 0.0, 0.0), (0.5, 0.15 * h, 0.4 * h, -0.3 * h, 10.0), (-0.3, 0.12 * h, -0.15 * h, 0.2 * h, -8.0)]
+    return ball_cone_projections(balls, ang, sad, cfg.n_det, n_rows)
