@@ -168,9 +168,14 @@ __device__ __forceinline__ void fft_pass(Cx<T>* buf, const Cx<T>* __restrict__ W
     __syncthreads();
 }
 
-// Registers: 16 complex points per thread are 32 (fp32) / 64 (fp64) registers; the bounds below hold the kernel to
-// 96 / 168 per thread (5 / 3 CTAs of 128 threads per SM) -- left alone the compiler hoists every table load of all
-// six passes and takes 220+ registers, i.e. two CTAs per SM.
+// Registers: 16 complex points per thread are 32 (fp32) / 64 (fp64) registers, and left alone the compiler hoists
+// the table loads of a whole pass and takes 220+.  What a cap buys depends on the block size:
+//   - N <= 2048 (blocks of <= 128 threads; configs 3 and 4): no cap.  Shared memory already limits these to <= 4
+//     CTAs per SM, a config-3 launch is 180 CTAs on 148 SMs, and every cap measured on B200 lost to none: the
+//     96-register build spilled 212 bytes in the passes (136-byte stack) and took 14.8 us for the config-3 filter,
+//     128 registers 13.2 us (still spilling), 255 registers 12.6 us with no local memory at all (whole step 42.3 ->
+//     40.1 us); the config-4 stack went 431 -> 413 us with half the resident warps.
+//   - longer transforms (256 / 512 threads) keep the caps below: 512 threads cannot have more than 128 registers.
 #ifndef FBP_FFT_REGS32
 #define FBP_FFT_REGS32 96
 #endif
@@ -179,7 +184,7 @@ __device__ __forceinline__ void fft_pass(Cx<T>* buf, const Cx<T>* __restrict__ W
 #endif
 template <typename T, int P> struct FftLaunch {
     static constexpr int threads = (1 << P) / 16 < 32 ? 32 : (1 << P) / 16;
-    static constexpr int regs = sizeof(T) == 4 ? FBP_FFT_REGS32 : FBP_FFT_REGS64;
+    static constexpr int regs = threads <= 128 ? 255 : (sizeof(T) == 4 ? FBP_FFT_REGS32 : FBP_FFT_REGS64);
     static constexpr int min_blocks = 65536 / (regs * threads) < 1 ? 1 : (65536 / (regs * threads) > 32 ? 32 : 65536 / (regs * threads));
 };
 
