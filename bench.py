@@ -394,6 +394,7 @@ def measure(args, dtype, world, rank, local, dist):
                   "metrics_ms": m_ms, "metrics_gbs": m_bytes / (m_ms * 1e-3) / 1e9, "metrics_bytes": m_bytes,
                   "psnr": float(out8[1].item()), "ssim": float(out8[2].item())}
 
+    issue_rate = fbp.fbp_measure_issue_rate(fbp.FBP_F32 if dtype == "f32" else fbp.FBP_F64)
     if world > 1:
         t = torch.tensor([ms_step, e2e_s, b_ms, f_ms], device="cuda", dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -404,7 +405,7 @@ def measure(args, dtype, world, rank, local, dist):
     return dict(info=info, graph_ms=graph_ms, ms_step=ms_step, f_ms=f_ms, b_ms=b_ms, e2e_s=e2e_s, updates=float(B) * N * N * K,
                 clocks=clk.summary(), esize=h_sino.element_size(),
                 h2d=h_sino.numel() * h_sino.element_size(), d2h=h_img.numel() * h_img.element_size(),
-                extras=extras, input_sha=input_sha)
+                extras=extras, input_sha=input_sha, issue_rate=issue_rate)
 
 
 def record(args, r, world, peaks, peaks_src, dtype):
@@ -443,9 +444,11 @@ def record(args, r, world, peaks, peaks_src, dtype):
         fma = cfg.batch * cfg.n_angles * ((2.0 * de * dn + cfg.n_det) if args.window == "ramlak" else float(cfg.n_det) ** 2)
         kern["filter_tfma_per_s"] = fma / (r["f_ms"] * 1e-3) / 1e12
         kern["filter_fma_frac_of_derived_peak"] = fma / (r["f_ms"] * 1e-3) / 1e12 / peak_tinstr
+    measured_tinstr = r.get("issue_rate", 0.0) / 1e12          # fbp_measure_issue_rate: FMA chains at full occupancy, this run
     roof = {"bound": "alu", "kernel": "backproject_kernel<%s>" % dtype, "achieved": achieved,
             "peak": peak_tinstr, "unit": "T %s lane-instr/s" % ("fp32" if dtype == "f32" else "fp64"),
             "frac": achieved / peak_tinstr,
+            "peak_measured": measured_tinstr, "frac_of_measured_peak": achieved / measured_tinstr if measured_tinstr > 0 else None,
             "traffic": ncu_traffic(args.config, dtype, "backproject"),
             "co_limit": {"bound": "smem", "achieved": smem_tbs, "peak": smem_peak_tbs, "unit": "TB/s of shared-memory operands",
                          "frac": smem_tbs / smem_peak_tbs,
@@ -454,8 +457,9 @@ def record(args, r, world, peaks, peaks_src, dtype):
                                  "column walk (FP64 pipe / issue bound; DESIGN.md 6.2)"
                                  % (smem_peak_tbs / smem_bytes_per_update / (peak_tinstr / FP_INSTR_PER_UPDATE))},
             "how": "%d FP instr/update (SURVEY 8(d)) x updates per launch / mean CUDA-event duration of the "
-                   "back-projection launch(es); peak = %d SMs x %d lanes x %.0f MHz (%s sm_max_mhz)"
-                   % (FP_INSTR_PER_UPDATE, n_sm, lanes, sm_max_mhz, peaks_src)}
+                   "back-projection launch(es); peak = %d SMs x %d lanes x %.0f MHz (%s sm_max_mhz); peak_measured = "
+                   "%.2f T lane-instr/s from the FMA issue-rate kernel of the library (fbp_measure_issue_rate) in this run"
+                   % (FP_INSTR_PER_UPDATE, n_sm, lanes, sm_max_mhz, peaks_src, measured_tinstr)}
     return {"value": total_updates / (r["ms_step"] * 1e-3) / 1e9, "ms_per_step": r["ms_step"],
             "slices_per_s": cfg.batch * world / (r["ms_step"] * 1e-3), "kernels": kern, "roofline": roof,
             "e2e": {"value": total_updates / r["e2e_s"] / 1e9, "unit": UNIT, "h2d_bytes_per_step": r["h2d"],

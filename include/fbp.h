@@ -329,6 +329,16 @@ fbp_status fbp_set_trace(fbp_plan *plan, unsigned long long *d_marks, long long 
 fbp_status fbp_set_profiling(fbp_plan *plan, int enable);
 fbp_status fbp_get_kernel_ms(fbp_plan *plan, float *filter_ms, float *backproject_ms);
 
+/*
+ * fbp_measure_issue_rate -- the FP32 (FFMA) or FP64 (DFMA) issue peak of the current device, measured: a kernel of
+ * independent FMA chains at full occupancy (two CTAs of 1024 threads per SM, 64 FMAs per loop trip), best of three
+ * timed launches after a warm-up, in lane-instructions per second (one FMA on one lane = 1).  This is the
+ * denominator bench.py states the back-projector's "alu" roofline against next to the figure derived from SM count,
+ * lanes and clock.  A measurement aid, not part of the reconstruction path:
+ * synchronous, runs on the legacy default stream, allocates and frees 16 bytes.  h_lane_instr_per_s: HOST pointer.
+ */
+fbp_status fbp_measure_issue_rate(fbp_dtype dtype, double *h_lane_instr_per_s);
+
 #ifdef __cplusplus
 }
 #endif

@@ -11,7 +11,7 @@ from .binding import (  # noqa: F401
     FbpError, load_library,
     fbp_create, fbp_create_tuned, OPTIONS, fbp_filter, fbp_backproject, fbp_reconstruct, fbp_reconstruct_host,
     fbp_destroy, fbp_last_error, fbp_plan_info, fbp_set_profiling, fbp_get_kernel_ms, fbp_set_trace, fbp_metrics, fbp_set_window, fbp_set_angle_weights, WINDOWS, fbp_interpolate_stack, fbp_project, fbp_fdk_reconstruct,
-    fbp_metrics_static, METRICS_STATIC_MAX_N,
+    fbp_metrics_static, METRICS_STATIC_MAX_N, fbp_measure_issue_rate,
 )
 from .build import build  # noqa: F401
 

@@ -19,7 +19,7 @@ EXPORTS = (
     "fbp_create", "fbp_create_tuned", "fbp_filter", "fbp_backproject", "fbp_reconstruct", "fbp_reconstruct_host",
     "fbp_destroy", "fbp_last_error", "fbp_plan_info", "fbp_set_profiling", "fbp_get_kernel_ms",
     "fbp_set_trace", "fbp_metrics", "fbp_set_window", "fbp_set_angle_weights", "fbp_interpolate_stack", "fbp_project", "fbp_fdk_reconstruct",
-    "fbp_metrics_static",
+    "fbp_metrics_static", "fbp_measure_issue_rate",
 )
 
 PLAN_INFO_FIELDS = (
@@ -70,6 +70,8 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     lib.fbp_metrics.restype = ci
     lib.fbp_metrics_static.argtypes = [ci, vp, vp, ctypes.c_longlong, cd, cd, cd, vp, vp]
     lib.fbp_metrics_static.restype = ci
+    lib.fbp_measure_issue_rate.argtypes = [ci, ctypes.POINTER(cd)]
+    lib.fbp_measure_issue_rate.restype = ci
     lib.fbp_set_window.argtypes = [vp, ci]
     lib.fbp_set_window.restype = ci
     lib.fbp_set_angle_weights.argtypes = [vp, ctypes.POINTER(cd)]
@@ -236,6 +238,14 @@ def fbp_metrics_static(dtype, d_x, d_y, n, max_val, c1, c2, d_out8, stream=None)
     lib = load_library()
     _check(lib, None, lib.fbp_metrics_static(int(dtype), _ptr(d_x), _ptr(d_y), int(n), float(max_val), float(c1),
                                              float(c2), _ptr(d_out8), _stream_handle(stream)))
+
+
+def fbp_measure_issue_rate(dtype) -> float:
+    """Measured FFMA / DFMA lane-instructions per second of the current device (include/fbp.h)."""
+    lib = load_library()
+    out = ctypes.c_double()
+    _check(lib, None, lib.fbp_measure_issue_rate(int(dtype), ctypes.byref(out)))
+    return out.value
 
 
 WINDOWS = {"ramlak": 0, "shepp-logan": 1, "cosine": 2, "hamming": 3, "hann": 4}

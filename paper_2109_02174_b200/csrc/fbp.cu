@@ -710,12 +710,15 @@ int pipe_group_size(const fbp_plan* p, int batch)
     return group < min_group ? min_group : group;
 }
 
-// fbp_reconstruct for a stack of slices: the filter is FMA-pipe bound and the back-projector
-// shared-memory bound, so they run well side by side.  The batch is cut into groups; group g+1 is
-// filtered on a plan-owned high-priority stream while group g is back-projected on one of two other
-// plan-owned streams (two, so that the tail of one launch overlaps the head of the next).  The
-// caller's stream forks into them and joins at the end: still enqueue-only, no host wait.  Same
-// kernels on the same data as the sequential path, hence the same bytes.
+// fbp_reconstruct for a stack of slices, group by group.  The batch is cut into groups; group g+1 is filtered on a
+// plan-owned high-priority stream while group g is back-projected on one of two other plan-owned streams (two, so
+// that the tail of one launch overlaps the head of the next).  The caller's stream forks into them and joins at the
+// end: still enqueue-only, no host wait.  Same kernels on the same data as the sequential path, hence the same bytes.
+// What it buys, measured on B200 at config 4 (64 slices): with HOST buffers (fbp_reconstruct_host) each group's
+// host-to-device copy rides the filter stream under the previous group's back-projection -- that is the case it is
+// kept for.  With device-resident data the FFT-form filter (shared-memory and latency bound, ~12 % of the step) and
+// the back-projector (shared-memory operand bound) compete for the same SMs and the step is within 1 % of the two
+// launches in sequence (profiles/r3_bench.md); it stays on there only so that both entry points run one code path.
 fbp_status run_pipelined(fbp_plan* p, const void* sino, void* image, int batch, cudaStream_t s,
                          const void* h_sino = nullptr)
 {
@@ -1459,3 +1462,65 @@ fbp_status fbp_metrics_static(fbp_dtype dtype, const void* d_x, const void* d_y,
 }
 
 }  // extern "C"
+
+// ---- fbp_measure_issue_rate: the denominator of the back-projector's roofline, measured ----------------------
+// Eight independent FMA chains per thread, 64 FMAs per loop trip, two CTAs of 1024 threads on every SM: nothing but
+// the FP32 (FFMA) or FP64 (DFMA) pipe limits it, so lane-instructions per second of this kernel is the issue peak
+// that bench.py's "alu" roofline is stated against ("builder measures with an FMA micro-benchmark").
+namespace fbp {
+template <typename T>
+__global__ void __launch_bounds__(1024) fma_rate_kernel(T* out, int iters, T a, T b)
+{
+    T x[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) x[q] = a + T(threadIdx.x + q);
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+#pragma unroll
+            for (int q = 0; q < 8; ++q) x[q] = fma(x[q], a, b);
+    }
+    T s = T(0);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) s += x[q];
+    if (s == T(-1)) out[0] = s;          // never true (a, b > 0): keeps the chains alive without a store per thread
+}
+}  // namespace fbp
+
+extern "C" fbp_status fbp_measure_issue_rate(fbp_dtype dtype, double* h_lane_instr_per_s)
+{
+    if (!h_lane_instr_per_s || (dtype != FBP_F32 && dtype != FBP_F64)) return fail(nullptr, FBP_EINVAL, "fbp_measure_issue_rate: bad arguments");
+    *h_lane_instr_per_s = 0.0;
+    int device = 0, sms = 0, major = 0;
+    cudaError_t e = cudaGetDevice(&device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "fbp_measure_issue_rate: device query");
+    if (major != 10) return fail(nullptr, FBP_EUNSUPPORTED, "libfbp is built for sm_100a (B200) only; no fallback path");
+    void* d_out = nullptr;
+    cudaEvent_t ev[2] = {nullptr, nullptr};
+    e = cudaMalloc(&d_out, 16);
+    if (e == cudaSuccess) e = cudaEventCreate(&ev[0]);
+    if (e == cudaSuccess) e = cudaEventCreate(&ev[1]);
+    const int grid = 2 * sms, iters = dtype == FBP_F32 ? 8192 : 4096;
+    float best_ms = 0.f;
+    for (int rep = 0; rep < 4 && e == cudaSuccess; ++rep) {          // rep 0 warms up (clocks, code)
+        e = cudaEventRecord(ev[0], nullptr);
+        if (e != cudaSuccess) break;
+        if (dtype == FBP_F32) fbp::fma_rate_kernel<float><<<grid, 1024>>>(static_cast<float*>(d_out), iters, 1.0000001f, 1e-7f);
+        else fbp::fma_rate_kernel<double><<<grid, 1024>>>(static_cast<double*>(d_out), iters, 1.0000001, 1e-7);
+        e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaEventRecord(ev[1], nullptr);
+        if (e == cudaSuccess) e = cudaEventSynchronize(ev[1]);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, ev[0], ev[1]);
+        if (e == cudaSuccess && rep > 0 && (best_ms == 0.f || ms < best_ms)) best_ms = ms;
+    }
+    if (ev[0]) cudaEventDestroy(ev[0]);
+    if (ev[1]) cudaEventDestroy(ev[1]);
+    cudaFree(d_out);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "fbp_measure_issue_rate");
+    if (!(best_ms > 0.f)) return fail(nullptr, FBP_ECUDA, "fbp_measure_issue_rate: no time measured");
+    *h_lane_instr_per_s = (double)grid * 1024.0 * (double)iters * 64.0 / ((double)best_ms * 1e-3);
+    return FBP_OK;
+}
