@@ -342,12 +342,17 @@ def measure(args, dtype, world, rank, local, dist):
     for _ in range(3):
         fbp.fbp_reconstruct_host(plan.handle, h_sino, h_img, B, stream)
     barrier()
+    # every call is timed on its own (fbp_reconstruct_host returns after the stream has drained): the median is the
+    # reported figure, min and max go beside it -- a mean hides a host that was busy for a few calls
     e2e_steps = max(3, min(args.steps, 100))
-    t0 = time.perf_counter()
+    e2e_each = []
     for _ in range(e2e_steps):
+        t0 = time.perf_counter()
         fbp.fbp_reconstruct_host(plan.handle, h_sino, h_img, B, stream)
+        e2e_each.append(time.perf_counter() - t0)
     barrier()
-    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    e2e_s = float(np.median(e2e_each))
+    e2e_spread = {"calls": e2e_steps, "ms_min": min(e2e_each) * 1e3, "ms_max": max(e2e_each) * 1e3, "ms_mean": float(np.mean(e2e_each)) * 1e3}
 
     extras = None
     if args.extras:
@@ -405,7 +410,7 @@ def measure(args, dtype, world, rank, local, dist):
     return dict(info=info, graph_ms=graph_ms, ms_step=ms_step, f_ms=f_ms, b_ms=b_ms, e2e_s=e2e_s, updates=float(B) * N * N * K,
                 clocks=clk.summary(), esize=h_sino.element_size(),
                 h2d=h_sino.numel() * h_sino.element_size(), d2h=h_img.numel() * h_img.element_size(),
-                extras=extras, input_sha=input_sha, issue_rate=issue_rate)
+                extras=extras, input_sha=input_sha, issue_rate=issue_rate, e2e_spread=e2e_spread)
 
 
 def record(args, r, world, peaks, peaks_src, dtype):
@@ -464,7 +469,8 @@ def record(args, r, world, peaks, peaks_src, dtype):
             "slices_per_s": cfg.batch * world / (r["ms_step"] * 1e-3), "kernels": kern, "roofline": roof,
             "e2e": {"value": total_updates / r["e2e_s"] / 1e9, "unit": UNIT, "h2d_bytes_per_step": r["h2d"],
                     "d2h_bytes_per_step": r["d2h"], "ms_per_step": r["e2e_s"] * 1e3,
-                    "api": "fbp_reconstruct_host (pinned host buffers, wall clock)"},
+                    "api": "fbp_reconstruct_host (pinned host buffers, wall clock; median of per-call times)",
+                    "spread": r["e2e_spread"]},
             "clocks": r["clocks"], "plan": info, "input_sha256": r["input_sha"],
             "graph_ms_per_step": r["graph_ms"]}
 
